@@ -1,0 +1,166 @@
+/*
+ * prand.h -- C ABI of the B200-native PRAND hot path (arXiv 1307.5869, Barash & Shchur).
+ *
+ * What the library does: it holds `n_streams` independent streams of one
+ * generator, initialised by block splitting -- stream s starts at position s*block_len of the single
+ * base sequence defined by the seed -- and fills a caller-owned DEVICE array with uniform numbers in
+ * the canonical interleaved layout
+ *
+ *        out[i * n_streams + s]  =  output number i (counted from the stream's current position)
+ *                                   of stream s,           0 <= i < n_per_stream, 0 <= s < n_streams.
+ *
+ * Every step (skip-operator application, the recurrences, conversion, stores) runs in hand-written
+ * CUDA kernels for sm_100a; there is no CPU fallback.  The host side only prepares the skip operators
+ * and launches.
+ *
+ * Conventions
+ *  - All functions return 0 (PRAND_OK) or a negative prand_error code; prand_strerror() names it.
+ *  - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Kernel
+ *    launches are asynchronous on it.  prand_init / prand_jump may synchronise it while uploading
+ *    operator tables; prand_get_state / prand_set_state / *_host synchronise.
+ *  - Pointers named `out` / `d_*` are DEVICE pointers, pointers named `host_*` are HOST pointers.
+ *  - The state object is opaque, lives on the device that was current in prand_init, and is owned by
+ *    the library until prand_free.  One state must not be used from two CUDA streams concurrently.
+ *  - Large distances are passed as mant * 2^log2 (the paper itself passes a*2^b to
+ *    mt19937_skipahead_, and split words to mrg32k3a_skipahead_).
+ *  - Position convention ("step-then-output"): a state at position P yields output number P by
+ *    advancing one step and reading the new state.
+ */
+#ifndef PRAND_H
+#define PRAND_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct prand_state prand_state;
+
+/* Generators (Table 2).  Numeric values are part of the ABI. */
+enum prand_gen {
+    PRAND_LFSR113 = 0,
+    PRAND_MRG32K3A = 1,
+    PRAND_MT19937 = 2,
+    PRAND_GM19 = 3,      /* PAPER.md:281-284, Table 2 */
+    PRAND_GM29 = 4,
+    PRAND_GM31 = 5,
+    PRAND_GM55 = 6,
+    PRAND_GM61 = 7,
+    PRAND_GQ58_1 = 8,
+    PRAND_GQ58_3 = 9,
+    PRAND_GQ58_4 = 10,
+    PRAND_NGEN = 11
+};
+
+enum prand_error {
+    PRAND_OK = 0,
+    PRAND_ERR_GEN = -1,        /* unknown generator id                                        */
+    PRAND_ERR_ARG = -2,        /* null pointer, n_streams == 0, mant == 0 with log2 != 0, ... */
+    PRAND_ERR_SEED = -3,       /* seed not valid for the generator (see prand_init)           */
+    PRAND_ERR_OVERFLOW = -4,   /* (first_stream + n_streams - 1) * mant does not fit 64 bits  */
+    PRAND_ERR_CUDA = -5,       /* a CUDA runtime call failed; prand_last_cuda_error() has it  */
+    PRAND_ERR_SIZE = -6,       /* byte count does not match prand_state_bytes()               */
+    PRAND_ERR_ALLOC = -7,      /* host or device allocation failed                            */
+    PRAND_ERR_INTERNAL = -8    /* self-check of a prepared operator failed                    */
+};
+
+/*
+ * prand_init -- block-splitting stream initialisation (rng_init_sequence_).
+ *   Creates `n_streams` streams of generator `gen`; stream s is the base sequence of `seed` advanced
+ *   s * block_len steps, block_len = block_len_mant * 2^block_len_log2 (block_len = 0 is allowed:
+ *   all streams identical).  Host: builds the skip operators for block_len * 2^j; device: one init
+ *   kernel applies them per stream and writes the structure-of-arrays state.
+ *   Seed convention: LFSR113 all four words = seed (invalid if any component's significant top bits
+ *   are zero, i.e. seed < 128); MRG32K3A all six words = seed (0 < seed < 2^32 - 22853); MT19937 the
+ *   ref.-[2] initialiser x_0 = seed, x_i = 1812433253 (x_{i-1} ^ (x_{i-1} >> 30)) + i; GM/GQ: base
+ *   orbit w(0) = 0, w(1) = seed mod g (must be non-zero), ensemble point i at orbit offset
+ *   (i+1) * 2^d (reading G3).  LFSR113/MRG32K3A/MT19937 seeds must be < 2^32.
+ *   `*st` receives the new state; on error it is set to NULL.
+ */
+int prand_init(prand_state **st, int gen, uint64_t seed, uint64_t n_streams,
+               uint64_t block_len_mant, unsigned block_len_log2, void *cuda_stream);
+
+/*
+ * prand_init_shard -- as prand_init, but this state holds only global streams
+ *   [first_stream, first_stream + n_streams) of the block-split family (multi-GPU sharding by stream
+ *   index; streams are independent, so no exchange is needed).  Local stream j is
+ *   global stream first_stream + j; the output layout is out[i * n_streams + j].
+ */
+int prand_init_shard(prand_state **st, int gen, uint64_t seed, uint64_t first_stream,
+                     uint64_t n_streams, uint64_t block_len_mant, unsigned block_len_log2,
+                     void *cuda_stream);
+
+/*
+ * prand_jump -- advance EVERY stream by steps = steps_mant * 2^steps_log2 without generating
+ *   (rng_skipahead_; PAPER.md:286-301, 347, 363-370, 374-378 for the algebra).
+ */
+int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_log2, void *cuda_stream);
+
+/*
+ * prand_generate_{u32,f32,f64} -- bulk generation (
+ *   rng_generate_gpu_array_{,float_,double_}).  `out` is device memory with n_per_stream * n_streams
+ *   elements, element-aligned; every stream advances n_per_stream.  Successive calls continue the
+ *   streams.  n_per_stream == 0 is a no-op.  There is no divisibility requirement (PAPER.md:404 had
+ *   one).  Internally a stream's range may be cut into sub-sections reached by jump-ahead
+ *   (PAPER.md:382); this never changes any output.
+ *     u32: the generator's 32-bit output word (MRG32K3A: z_n in [0, 2^32-209)).
+ *     f32: (u >> 8) * 2^-24 in [0,1)   (reading CONV).
+ *     f64: u * 2^-32 in [0,1); MRG32K3A: (z_n ? z_n : m1) / (m1 + 1) in (0,1) (reading M3).
+ */
+int prand_generate_u32(prand_state *st, uint32_t *out, uint64_t n_per_stream, void *cuda_stream);
+int prand_generate_f32(prand_state *st, float *out, uint64_t n_per_stream, void *cuda_stream);
+int prand_generate_f64(prand_state *st, double *out, uint64_t n_per_stream, void *cuda_stream);
+
+/*
+ * prand_generate_{u32,f32,f64}_host -- the same numbers delivered to HOST memory
+ *   (rng_generate_array_): generated on the device in row blocks and copied back with
+ *   overlapping device-to-host copies.  `host_out` has n_per_stream * n_streams elements (pinned
+ *   memory gives full PCIe speed; pageable memory works).  Returns after the data has arrived.
+ */
+int prand_generate_u32_host(prand_state *st, uint32_t *host_out, uint64_t n_per_stream, void *cuda_stream);
+int prand_generate_f32_host(prand_state *st, float *host_out, uint64_t n_per_stream, void *cuda_stream);
+int prand_generate_f64_host(prand_state *st, double *host_out, uint64_t n_per_stream, void *cuda_stream);
+
+/*
+ * Canonical state export / import (the state is plain data and may be copied between
+ * host and device; generation continues from it).  Per stream, little-endian, streams consecutive:
+ *   LFSR113   4 x u32  z1..z4 masked to their significant top 31/29/28/25 bits;
+ *   MRG32K3A  6 x u32  x_n, x_{n-1}, x_{n-2}, y_n, y_{n-1}, y_{n-2};
+ *   MT19937   624 x u32 window x_P..x_{P+623}, low 31 bits of word 0 zeroed;
+ *   GM/GQ     2s words xP_0, xN_0, ..., xP_{s-1}, xN_{s-1} (u32 if g < 2^32, else u64), residues mod g.
+ * prand_state_bytes() = n_streams * per-stream bytes.  Both calls synchronise the device.
+ */
+size_t prand_state_bytes(const prand_state *st);
+int prand_get_state(const prand_state *st, void *host_buf, size_t bytes);
+int prand_set_state(prand_state *st, const void *host_buf, size_t bytes);
+
+uint64_t prand_n_streams(const prand_state *st);
+int prand_gen_of(const prand_state *st);
+
+/* Releases the state and every device buffer it owns (synchronises the device first). */
+int prand_free(prand_state *st);
+
+/*
+ * prand_fill_u32 -- write-peak probe: 128-bit stores of a constant to `n_words` u32 at device
+ *   pointer `out` (16-byte aligned).  Used by the bench to measure the HBM write roofline in the
+ *   same run as the generators.
+ */
+int prand_fill_u32(uint32_t *out, uint64_t n_words, uint32_t value, void *cuda_stream);
+
+/* Number of kernels this library has launched in this process (for bench.py's gpu_launches). */
+uint64_t prand_launch_count(void);
+
+/* Name of the kernel configuration the last generate call on `st` used (static string). */
+const char *prand_last_kernel(const prand_state *st);
+
+const char *prand_strerror(int code);
+/* cudaError_t of the last failing CUDA call in this thread (0 if none). */
+int prand_last_cuda_error(void);
+const char *prand_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PRAND_H */

@@ -1,0 +1,79 @@
+// internal.h -- types shared by the host-side preparation (prand.cu) and the kernel files.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/prand.h"
+
+namespace prand {
+
+enum { DT_U32 = 0, DT_F32 = 1, DT_F64 = 2 };
+
+// ---- skip operators (a0 builds them on the host, the kernels apply them) -------------------------
+// LFSR113: one step of a component is GF(2)-linear on its 32-bit word;
+// col[c][j] = image of the unit word 1<<j under the n-step map of component c.
+struct LfsrOp { uint32_t col[4][32]; };
+// MRG32K3A: A^n mod m1, B^n mod m2, row-major 3x3 residues.
+struct MrgOp { uint32_t a[9]; uint32_t b[9]; };
+// GM/GQ: n-th power of the companion matrix [[k,-q],[1,0]] mod g, row-major,
+// acting on the column (x^(n), x^(n-1)) = (xN, xP).
+struct GmOp { uint64_t m[4]; };
+// MT19937: g_v(x) = x^v mod phi(x) (eq. 10); bit (i & 31) of w[i >> 5] = a_i.
+struct MtOp { uint32_t w[624]; };
+
+// GM/GQ parameters, Table 2 + Table 5 ensemble sizes.
+struct GmParams {
+    uint64_t k, q, g;
+    unsigned v, s, d;      // output bits per point, ensemble size, log2 of the orbit spacing D
+    unsigned nbits;        // bit length of g
+    uint64_t mu;           // floor(2^(2 nbits) / g) for Barrett reduction in the jump kernels
+    bool wide;             // state words are u64 (g >= 2^32)
+};
+const GmParams *gm_params(int gen);   // nullptr if gen is not a GM/GQ generator
+
+// How a jump kernel finds the exponent of stream j: idx = idx0 + j * idx_stride; the operator
+// applied is prod_{bit b of idx set} ops[b].  base != nullptr: start from the broadcast base state
+// instead of st_in (stream initialisation).
+struct JumpArgs {
+    const void *base;
+    const void *st_in;
+    void *st_out;
+    uint64_t n_streams;
+    const void *ops;       // device array of per-level operators
+    uint64_t idx0, idx_stride;
+};
+
+// One bulk generation launch.  Rows [0, n) of every stream; when n_chunks > 1 virtual stream
+// (s, c) first jumps c * chunk_len ahead with chunk_ops (levels = bits of c) and fills rows
+// [c*chunk_len, min(n, (c+1)*chunk_len)); the last chunk writes the final state to st_out.
+struct GenArgs {
+    const void *st_in;
+    void *st_out;
+    void *out;
+    int dtype;
+    uint64_t n_streams;
+    uint64_t n;
+    uint64_t chunk_len;
+    uint64_t n_chunks;
+    const void *chunk_ops;
+};
+
+struct LaunchInfo { const char *kernel; unsigned launches; };
+
+cudaError_t lfsr113_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
+cudaError_t lfsr113_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
+cudaError_t mrg32k3a_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
+cudaError_t mrg32k3a_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
+cudaError_t gm_jump(cudaStream_t, int gen, const JumpArgs &, LaunchInfo *);
+cudaError_t gm_generate(cudaStream_t, int gen, const GenArgs &, LaunchInfo *);
+// MT19937: dst stream j (j in [dst0, dst0+count)) = g(A) applied to src stream (j - src_back), or to
+// itself when src_back == 0.  State layout [stream][624].
+cudaError_t mt19937_apply(cudaStream_t, const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
+                          uint64_t count, uint64_t src_back, const MtOp *d_op, LaunchInfo *);
+cudaError_t mt19937_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
+cudaError_t fill_u32(cudaStream_t, uint32_t *out, uint64_t n_words, uint32_t value, LaunchInfo *);
+
+int sm_count();   // cached multiprocessor count of the current device
+
+}  // namespace prand

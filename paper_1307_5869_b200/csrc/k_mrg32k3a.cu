@@ -1,0 +1,200 @@
+// k_mrg32k3a.cu -- MRG32K3A jump and generation kernels.
+//
+// PAPER.md:336-347 (eqs. 5-6): X_{n+1} = A X_n mod m1, Y_{n+1} = B Y_n mod m2 with
+//   x_{n+1} = a x_{n-1} + b x_{n-2} mod m1,  a = 1403580, b = -810728,  m1 = 2^32 - 209,
+//   y_{n+1} = c y_n     + d y_{n-2} mod m2,  c = 527612,  d = -1370589, m2 = 2^32 - 22853.
+// Output (reading M1): z_n = (x_n - y_n) mod m1; f64 = (z_n ? z_n : m1) * 1/(m1+1) (M3).
+// Reduction uses 2^32 = 209 (mod m1) and 2^32 = 22853 (mod m2): fold the high word down twice.
+// State layout (SoA): word w of stream s at st[w * n_streams + s], w = x_n, x_{n-1}, x_{n-2},
+// y_n, y_{n-1}, y_{n-2}.
+#include "k_common.cuh"
+
+namespace prand {
+namespace {
+
+constexpr uint32_t M1 = 4294967087u, M2 = 4294944443u;
+constexpr uint32_t C1 = 209u, C2 = 22853u;
+
+// t < 2^54  ->  t mod m1
+__device__ __forceinline__ uint32_t reduce_m1(uint64_t t)
+{
+    uint64_t u = (uint64_t)(uint32_t)(t >> 32) * C1 + (uint32_t)t;   // < 2^22*209 + 2^32 < 2^32 + 2^30
+    uint32_t lo = (uint32_t)u;
+    uint32_t r = lo + (uint32_t)(u >> 32) * C1;                      // hi in {0,1}; no wrap when hi = 1
+    return r >= M1 ? r - M1 : r;
+}
+// t < 2^54  ->  t mod m2
+__device__ __forceinline__ uint32_t reduce_m2(uint64_t t)
+{
+    uint64_t u = (uint64_t)(uint32_t)(t >> 32) * C2 + (uint32_t)t;   // < 2^22*22853 + 2^32 < 2^37
+    uint64_t w = (uint64_t)(uint32_t)(u >> 32) * C2 + (uint32_t)u;   // < 2^5*22853 + 2^32 < 2 m2
+    return (uint32_t)(w >= M2 ? w - M2 : w);
+}
+
+struct Mrg { uint32_t x0, x1, x2, y0, y1, y2; };   // x0 = x_n, x1 = x_{n-1}, x2 = x_{n-2}
+
+__device__ __forceinline__ uint32_t mrg_step(Mrg &s)
+{
+    uint64_t tx = (uint64_t)1403580u * s.x1 + (uint64_t)810728u * (M1 - s.x2);
+    uint64_t ty = (uint64_t)527612u * s.y0 + (uint64_t)1370589u * (M2 - s.y2);
+    uint32_t nx = reduce_m1(tx), ny = reduce_m2(ty);
+    s.x2 = s.x1; s.x1 = s.x0; s.x0 = nx;
+    s.y2 = s.y1; s.y1 = s.y0; s.y0 = ny;
+    // z = (x - y) mod m1 with x < m1, y < m2 (y may be >= m1 by at most m2 - m1 < m1)
+    uint32_t yy = ny >= M1 ? ny - M1 : ny;
+    return nx >= yy ? nx - yy : nx + (M1 - yy);
+}
+
+template <int DT> __device__ __forceinline__ typename OutElem<DT>::type mrg_convert(uint32_t z)
+{
+    if constexpr (DT == DT_F64) {
+        // one IEEE double multiply of an exactly converted integer (reading M3)
+        return (double)(z == 0 ? M1 : z) * 2.328306549295727688e-10;
+    } else {
+        return convert<DT>(z);
+    }
+}
+
+// generic a*b mod m for the (cold) jump path: a, b < m = 2^32 - cfold
+__device__ __forceinline__ uint32_t mulmod32(uint32_t a, uint32_t b, uint32_t m, uint32_t cfold)
+{
+    uint64_t t = (uint64_t)a * b;
+    for (int k = 0; k < 3; k++) t = (t >> 32) * cfold + (uint32_t)t;   // < 2^32 + cfold after 3 folds
+    while (t >= m) t -= m;
+    return (uint32_t)t;
+}
+__device__ __forceinline__ uint32_t addmod32(uint32_t a, uint32_t b, uint32_t m)
+{
+    uint64_t t = (uint64_t)a + b;
+    return (uint32_t)(t >= m ? t - m : t);
+}
+__device__ __forceinline__ void matvec3(const uint32_t *__restrict__ mt, uint32_t &v0, uint32_t &v1,
+                                        uint32_t &v2, uint32_t m, uint32_t cfold)
+{
+    uint32_t r[3];
+    for (int i = 0; i < 3; i++) {
+        uint32_t acc = mulmod32(__ldg(mt + 3 * i), v0, m, cfold);
+        acc = addmod32(acc, mulmod32(__ldg(mt + 3 * i + 1), v1, m, cfold), m);
+        acc = addmod32(acc, mulmod32(__ldg(mt + 3 * i + 2), v2, m, cfold), m);
+        r[i] = acc;
+    }
+    v0 = r[0]; v1 = r[1]; v2 = r[2];
+}
+__device__ __forceinline__ void mrg_apply_bits(const MrgOp *__restrict__ ops, uint64_t idx, Mrg &s)
+{
+    for (int lev = 0; idx != 0; lev++, idx >>= 1)
+        if (idx & 1) {
+            matvec3(ops[lev].a, s.x0, s.x1, s.x2, M1, C1);
+            matvec3(ops[lev].b, s.y0, s.y1, s.y2, M2, C2);
+        }
+}
+
+__device__ __forceinline__ Mrg mrg_load(const uint32_t *st, uint64_t ns, uint64_t s)
+{
+    Mrg r;
+    r.x0 = st[s]; r.x1 = st[ns + s]; r.x2 = st[2 * ns + s];
+    r.y0 = st[3 * ns + s]; r.y1 = st[4 * ns + s]; r.y2 = st[5 * ns + s];
+    return r;
+}
+__device__ __forceinline__ void mrg_store(uint32_t *st, uint64_t ns, uint64_t s, const Mrg &r)
+{
+    st[s] = r.x0; st[ns + s] = r.x1; st[2 * ns + s] = r.x2;
+    st[3 * ns + s] = r.y0; st[4 * ns + s] = r.y1; st[5 * ns + s] = r.y2;
+}
+
+__global__ void __launch_bounds__(256)
+mrg32k3a_jump_kernel(const uint32_t *__restrict__ base, const uint32_t *st_in,
+                     uint32_t *st_out, uint64_t ns, const MrgOp *__restrict__ ops,
+                     uint64_t idx0, uint64_t idx_stride)
+{
+    uint64_t s = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= ns) return;
+    Mrg r;
+    if (base) { r.x0 = base[0]; r.x1 = base[1]; r.x2 = base[2]; r.y0 = base[3]; r.y1 = base[4]; r.y2 = base[5]; }
+    else r = mrg_load(st_in, ns, s);
+    mrg_apply_bits(ops, idx0 + s * idx_stride, r);
+    mrg_store(st_out, ns, s, r);
+}
+
+// One thread owns V adjacent streams and one row chunk (see k_lfsr113.cu for the mapping).
+template <int V, int DT>
+__global__ void __launch_bounds__(256)
+mrg32k3a_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
+                    typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n,
+                    uint64_t chunk_len, uint64_t n_chunks, const MrgOp *__restrict__ chunk_ops)
+{
+    typedef typename OutElem<DT>::type T;
+    const uint64_t groups = ns / V;
+    const uint64_t vid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (vid >= groups * n_chunks) return;
+    const uint64_t c = vid / groups, sg = vid - c * groups;
+    const uint64_t s0 = sg * V;
+
+    Mrg g[V];
+#pragma unroll
+    for (int v = 0; v < V; v++) g[v] = mrg_load(st_in, ns, s0 + v);
+    if (c != 0) {
+#pragma unroll
+        for (int v = 0; v < V; v++) mrg_apply_bits(chunk_ops, c, g[v]);
+    }
+    const uint64_t row0 = c * chunk_len;
+    const uint64_t row1 = (row0 + chunk_len < n) ? row0 + chunk_len : n;
+    T *p = out + row0 * ns + s0;
+#pragma unroll 2
+    for (uint64_t i = row0; i < row1; i++) {
+        T r[V];
+#pragma unroll
+        for (int v = 0; v < V; v++) r[v] = mrg_convert<DT>(mrg_step(g[v]));
+        store_vec<V>(p, r);
+        p += ns;
+    }
+    if (c == n_chunks - 1) {
+#pragma unroll
+        for (int v = 0; v < V; v++) mrg_store(st_out, ns, s0 + v, g[v]);
+    }
+}
+
+template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
+{
+    typedef typename OutElem<DT>::type T;
+    uint64_t threads = (a.n_streams / V) * a.n_chunks;
+    unsigned blocks = (unsigned)ceil_div_u64(threads, 256);
+    mrg32k3a_gen_kernel<V, DT><<<blocks, 256, 0, stream>>>(
+        (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
+        a.n_chunks, (const MrgOp *)a.chunk_ops);
+    return cudaGetLastError();
+}
+
+template <int DT> cudaError_t dispatch_v(cudaStream_t stream, const GenArgs &a, LaunchInfo *li)
+{
+    constexpr int VMAX = (DT == DT_F64) ? 2 : 4;   // one 128-bit store per row
+    bool vec = (a.n_streams % VMAX == 0) && ((uintptr_t)a.out % 16 == 0);
+    li->launches = 1;
+    if (vec) { li->kernel = (DT == DT_F64) ? "mrg32k3a_gen<V=2>" : "mrg32k3a_gen<V=4>"; return launch_gen<VMAX, DT>(stream, a); }
+    li->kernel = "mrg32k3a_gen<V=1>";
+    return launch_gen<1, DT>(stream, a);
+}
+
+}  // namespace
+
+cudaError_t mrg32k3a_jump(cudaStream_t stream, const JumpArgs &a, LaunchInfo *li)
+{
+    unsigned blocks = (unsigned)ceil_div_u64(a.n_streams, 256);
+    mrg32k3a_jump_kernel<<<blocks, 256, 0, stream>>>((const uint32_t *)a.base, (const uint32_t *)a.st_in,
+                                                     (uint32_t *)a.st_out, a.n_streams,
+                                                     (const MrgOp *)a.ops, a.idx0, a.idx_stride);
+    li->kernel = "mrg32k3a_jump";
+    li->launches = 1;
+    return cudaGetLastError();
+}
+
+cudaError_t mrg32k3a_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *li)
+{
+    switch (a.dtype) {
+    case DT_U32: return dispatch_v<DT_U32>(stream, a, li);
+    case DT_F32: return dispatch_v<DT_F32>(stream, a, li);
+    default: return dispatch_v<DT_F64>(stream, a, li);
+    }
+}
+
+}  // namespace prand

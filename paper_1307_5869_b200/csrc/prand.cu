@@ -1,0 +1,739 @@
+// prand.cu -- the C-ABI boundary of libprand (include/prand.h, include/prand_host.h): argument
+// checks, host preparation of the skip operators (a0, skip_ops.cpp), state management, launch policy
+// and the calls into the kernel files.  Every arithmetic step of the hot path runs in the kernels;
+// there is no CPU fallback.  Product code: shares nothing with oracle/.
+#include <atomic>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+#include "internal.h"
+#include "skip_ops.h"
+#include "../../include/prand_host.h"
+
+using namespace prand;
+using prand::host::Dist;
+
+// ---- generator tables -----------------------------------------------------------------------------
+namespace prand {
+
+static GmParams make_gm(uint64_t k, uint64_t q, uint64_t g, unsigned v, unsigned s, unsigned d)
+{
+    GmParams p;
+    p.k = k; p.q = q; p.g = g; p.v = v; p.s = s; p.d = d;
+    p.nbits = 64 - (unsigned)__builtin_clzll(g);
+    p.mu = (uint64_t)((((unsigned __int128)1) << (2 * p.nbits)) / g);
+    p.wide = g >= (1ull << 32);
+    return p;
+}
+
+// Table 2: k, q, g, v; Table 5: ensemble size s; d: reading G3.
+const GmParams *gm_params(int gen)
+{
+    static const GmParams tab[8] = {
+        make_gm(15, 28, (1ull << 19) - 1, 1, 32, 32),                          // GM19
+        make_gm(4, 2, (1ull << 29) - 3, 1, 32, 52),                            // GM29
+        make_gm(11, 14, (1ull << 31) - 1, 1, 32, 56),                          // GM31
+        make_gm(256, 176, 16ull * ((1ull << 51) - 129), 4, 8, 98),             // GM55
+        make_gm(24, 74, (1ull << 61) - 1, 1, 32, 116),                         // GM61
+        make_gm(8, 48, ((1ull << 29) - 3) << 29, 1, 32, 52),                   // GQ58.1
+        make_gm(8, 48, ((1ull << 29) - 3) << 29, 3, 12, 54),                   // GQ58.3
+        make_gm(8, 48, ((1ull << 29) - 3) << 29, 4, 8, 54),                    // GQ58.4
+    };
+    if (gen < PRAND_GM19 || gen > PRAND_GQ58_4) return nullptr;
+    return &tab[gen - PRAND_GM19];
+}
+
+int sm_count()
+{
+    static int cached_dev = -1, cached = 0;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 148;
+    if (dev != cached_dev) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        cached = n;
+        cached_dev = dev;
+    }
+    return cached;
+}
+
+}  // namespace prand
+
+namespace {
+
+std::atomic<uint64_t> g_launches{0};
+thread_local int g_last_cuda_error = 0;
+
+inline bool is_gm(int gen) { return gen >= PRAND_GM19 && gen <= PRAND_GQ58_4; }
+
+// words per stream and bytes per word of the state (internal SoA and canonical export agree on both)
+inline size_t state_words(int gen)
+{
+    if (gen == PRAND_LFSR113) return 4;
+    if (gen == PRAND_MRG32K3A) return 6;
+    if (gen == PRAND_MT19937) return host::MT_N;
+    if (const GmParams *p = gm_params(gen)) return 2 * (size_t)p->s;
+    return 0;
+}
+inline size_t state_word_bytes(int gen)
+{
+    const GmParams *p = gm_params(gen);
+    return (p && p->wide) ? 8 : 4;
+}
+inline size_t stream_bytes(int gen) { return state_words(gen) * state_word_bytes(gen); }
+
+inline unsigned bit_length(uint64_t x) { return x ? 64u - (unsigned)__builtin_clzll(x) : 0u; }
+
+int cuda_fail(cudaError_t e)
+{
+    g_last_cuda_error = (int)e;
+    return PRAND_ERR_CUDA;
+}
+#define CU(call)                                         \
+    do {                                                 \
+        cudaError_t e_ = (call);                         \
+        if (e_ != cudaSuccess) return cuda_fail(e_);     \
+    } while (0)
+
+}  // namespace
+
+struct prand_state {
+    int gen;
+    int device;
+    uint64_t ns;            // streams held by this state
+    uint64_t first;         // global index of local stream 0
+    void *d_state[2];       // [cur] holds the streams; the other one is the target of chunked launches
+    int cur;
+    size_t bytes;           // ns * stream_bytes(gen)
+    void *d_ops;            // scratch for uploaded operator tables (grown on demand)
+    size_t ops_bytes;
+    void *d_chunk_ops;      // cached operators for chunk_len * 2^j
+    uint64_t chunk_len;
+    unsigned chunk_levels;
+    void *d_stage[2];       // device staging of the *_host calls
+    size_t stage_bytes;
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_gen[2], ev_copy[2];
+    bool host_ready;
+    const char *last_kernel;
+};
+
+namespace {
+
+int ensure_ops(prand_state *st, size_t bytes)
+{
+    if (bytes <= st->ops_bytes) return PRAND_OK;
+    if (st->d_ops) { CU(cudaDeviceSynchronize()); CU(cudaFree(st->d_ops)); st->d_ops = nullptr; st->ops_bytes = 0; }
+    CU(cudaMalloc(&st->d_ops, bytes));
+    st->ops_bytes = bytes;
+    return PRAND_OK;
+}
+
+int ensure_second_buffer(prand_state *st)
+{
+    if (st->d_state[1 - st->cur]) return PRAND_OK;
+    CU(cudaMalloc(&st->d_state[1 - st->cur], st->bytes));
+    return PRAND_OK;
+}
+
+void note(prand_state *st, const LaunchInfo &li)
+{
+    g_launches.fetch_add(li.launches, std::memory_order_relaxed);
+    if (st) st->last_kernel = li.kernel;
+}
+
+// Host operators for distance n * 2^j, j < levels, as a flat byte vector in the kernels' layout.
+int build_level_ops(int gen, Dist n, unsigned levels, std::vector<unsigned char> &bytes)
+{
+    if (gen == PRAND_LFSR113) {
+        std::vector<LfsrOp> v;
+        host::lfsr113_levels(n, levels, v);
+        bytes.assign((unsigned char *)v.data(), (unsigned char *)(v.data() + v.size()));
+    } else if (gen == PRAND_MRG32K3A) {
+        std::vector<MrgOp> v;
+        host::mrg32k3a_levels(n, levels, v);
+        bytes.assign((unsigned char *)v.data(), (unsigned char *)(v.data() + v.size()));
+    } else if (is_gm(gen)) {
+        std::vector<GmOp> v;
+        host::gm_levels(*gm_params(gen), n, levels, v);
+        bytes.assign((unsigned char *)v.data(), (unsigned char *)(v.data() + v.size()));
+    } else if (gen == PRAND_MT19937) {
+        std::vector<host::MtPoly> v;
+        host::mt19937_levels(n, levels, v);
+        std::vector<MtOp> ops(v.size());
+        for (size_t i = 0; i < v.size(); i++) host::mt19937_to_op(v[i], ops[i]);
+        bytes.assign((unsigned char *)ops.data(), (unsigned char *)(ops.data() + ops.size()));
+    } else {
+        return PRAND_ERR_GEN;
+    }
+    return PRAND_OK;
+}
+
+// Canonical seed state of one stream (not masked), words of state_word_bytes(gen).
+int build_seed_state(int gen, uint64_t seed, std::vector<unsigned char> &bytes)
+{
+    bytes.assign(stream_bytes(gen), 0);
+    if (gen == PRAND_LFSR113) {
+        // all four words = seed; a component whose significant top bits vanish stays zero forever
+        if (seed > 0xFFFFFFFFull || (seed & 0xFFFFFF80ull) == 0) return PRAND_ERR_SEED;
+        uint32_t *w = (uint32_t *)bytes.data();
+        for (int c = 0; c < 4; c++) w[c] = (uint32_t)seed;
+    } else if (gen == PRAND_MRG32K3A) {
+        if (seed == 0 || seed >= 4294944443ull) return PRAND_ERR_SEED;
+        uint32_t *w = (uint32_t *)bytes.data();
+        for (int c = 0; c < 6; c++) w[c] = (uint32_t)seed;
+    } else if (gen == PRAND_MT19937) {
+        if (seed > 0xFFFFFFFFull) return PRAND_ERR_SEED;
+        host::mt19937_seed_state((uint32_t)seed, (uint32_t *)bytes.data());
+    } else if (const GmParams *p = gm_params(gen)) {
+        uint64_t words[64];
+        if (!host::gm_seed_state(*p, seed, words)) return PRAND_ERR_SEED;
+        for (unsigned i = 0; i < 2 * p->s; i++) {
+            if (p->wide) ((uint64_t *)bytes.data())[i] = words[i];
+            else ((uint32_t *)bytes.data())[i] = (uint32_t)words[i];
+        }
+    } else {
+        return PRAND_ERR_GEN;
+    }
+    return PRAND_OK;
+}
+
+cudaError_t launch_jump(cudaStream_t stream, int gen, const JumpArgs &a, LaunchInfo *li)
+{
+    if (gen == PRAND_LFSR113) return lfsr113_jump(stream, a, li);
+    if (gen == PRAND_MRG32K3A) return mrg32k3a_jump(stream, a, li);
+    return gm_jump(stream, gen, a, li);
+}
+
+}  // namespace
+
+// ==================================================================================================
+// prand_init / prand_init_shard (a0 + a1)
+// ==================================================================================================
+namespace {
+
+// MT19937: stream 0 of the shard = seed window jumped first * L; then a doubling tree -- level j
+// fills local streams [2^j, 2^(j+1)) from [0, 2^j) with g_{L 2^j} (eq. 10), one application each.
+int init_mt19937(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
+{
+    const unsigned lev_all = bit_length(st->first + st->ns - 1);
+    const unsigned lev_tree = bit_length(st->ns - 1);
+    std::vector<unsigned char> base;
+    int rc = build_seed_state(PRAND_MT19937, seed, base);
+    if (rc) return rc;
+    std::vector<host::MtPoly> polys;
+    host::mt19937_levels(L, lev_all, polys);
+    std::vector<MtOp> ops(lev_tree + 1);
+    for (unsigned j = 0; j < lev_tree; j++) host::mt19937_to_op(polys[j], ops[j]);
+    bool have_first = false;
+    if (st->first) {                                   // x^(first L) = product of the levels of first's bits
+        host::MtPoly acc;
+        for (unsigned j = 0; j < lev_all; j++) {
+            if (!((st->first >> j) & 1)) continue;
+            if (!have_first) { acc = polys[j]; have_first = true; }
+            else host::mt19937_mulmod(acc, acc, polys[j]);
+        }
+        host::mt19937_to_op(acc, ops[lev_tree]);
+    }
+    rc = ensure_ops(st, ops.size() * sizeof(MtOp));
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(st->d_ops, ops.data(), ops.size() * sizeof(MtOp), cudaMemcpyHostToDevice, stream));
+    uint32_t *d = (uint32_t *)st->d_state[st->cur];
+    CU(cudaMemcpyAsync(d, base.data(), base.size(), cudaMemcpyHostToDevice, stream));
+    const MtOp *d_ops = (const MtOp *)st->d_ops;
+    LaunchInfo li;
+    if (have_first) {
+        CU(mt19937_apply(stream, d, d, 0, 1, 0, d_ops + lev_tree, &li));
+        note(st, li);
+    }
+    for (unsigned j = 0; j < lev_tree; j++) {
+        uint64_t lo = 1ull << j;
+        uint64_t count = st->ns - lo < lo ? st->ns - lo : lo;
+        CU(mt19937_apply(stream, d, d, lo, count, lo, d_ops + j, &li));
+        note(st, li);
+    }
+    return PRAND_OK;
+}
+
+int init_body(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
+{
+    if (st->gen == PRAND_MT19937) return init_mt19937(st, seed, L, stream);
+    std::vector<unsigned char> base, ops;
+    int rc = build_seed_state(st->gen, seed, base);
+    if (rc) return rc;
+    const unsigned levels = bit_length(st->first + st->ns - 1);
+    rc = build_level_ops(st->gen, L, levels, ops);
+    if (rc) return rc;
+    const size_t ops_off = (base.size() + 255) & ~(size_t)255;
+    rc = ensure_ops(st, ops_off + ops.size() + 256);
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(st->d_ops, base.data(), base.size(), cudaMemcpyHostToDevice, stream));
+    if (!ops.empty())
+        CU(cudaMemcpyAsync((char *)st->d_ops + ops_off, ops.data(), ops.size(), cudaMemcpyHostToDevice, stream));
+    JumpArgs a;
+    a.base = st->d_ops;
+    a.st_in = nullptr;
+    a.st_out = st->d_state[st->cur];
+    a.n_streams = st->ns;
+    a.ops = (char *)st->d_ops + ops_off;
+    a.idx0 = st->first;
+    a.idx_stride = 1;
+    LaunchInfo li;
+    CU(launch_jump(stream, st->gen, a, &li));
+    note(st, li);
+    return PRAND_OK;
+}
+
+void destroy(prand_state *st)
+{
+    if (!st) return;
+    cudaDeviceSynchronize();
+    for (int i = 0; i < 2; i++) {
+        if (st->d_state[i]) cudaFree(st->d_state[i]);
+        if (st->d_stage[i]) cudaFree(st->d_stage[i]);
+        if (st->host_ready) { cudaEventDestroy(st->ev_gen[i]); cudaEventDestroy(st->ev_copy[i]); }
+    }
+    if (st->host_ready) cudaStreamDestroy(st->copy_stream);
+    if (st->d_ops) cudaFree(st->d_ops);
+    if (st->d_chunk_ops) cudaFree(st->d_chunk_ops);
+    delete st;
+}
+
+}  // namespace
+
+extern "C" int prand_init_shard(prand_state **out, int gen, uint64_t seed, uint64_t first_stream,
+                                uint64_t n_streams, uint64_t block_len_mant, unsigned block_len_log2,
+                                void *cuda_stream)
+{
+    if (!out) return PRAND_ERR_ARG;
+    *out = nullptr;
+    if (gen < 0 || gen >= PRAND_NGEN) return PRAND_ERR_GEN;
+    if (n_streams == 0) return PRAND_ERR_ARG;
+    if (block_len_mant == 0 && block_len_log2 != 0) return PRAND_ERR_ARG;
+    if (block_len_log2 > 4096) return PRAND_ERR_ARG;
+    if (first_stream + n_streams < first_stream) return PRAND_ERR_OVERFLOW;
+    {
+        unsigned __int128 top = (unsigned __int128)(first_stream + n_streams - 1) * block_len_mant;
+        if (top >> 64) return PRAND_ERR_OVERFLOW;
+    }
+    {   // seed validity before any allocation
+        std::vector<unsigned char> tmp;
+        int rc = build_seed_state(gen, seed, tmp);
+        if (rc) return rc;
+    }
+    prand_state *st = new (std::nothrow) prand_state();
+    if (!st) return PRAND_ERR_ALLOC;
+    std::memset(st, 0, sizeof *st);
+    st->gen = gen;
+    st->ns = n_streams;
+    st->first = first_stream;
+    st->bytes = (size_t)n_streams * stream_bytes(gen);
+    st->last_kernel = "";
+    cudaError_t e = cudaGetDevice(&st->device);
+    if (e == cudaSuccess) e = cudaMalloc(&st->d_state[0], st->bytes);
+    if (e != cudaSuccess) {
+        delete st;
+        g_last_cuda_error = (int)e;
+        return e == cudaErrorMemoryAllocation ? PRAND_ERR_ALLOC : PRAND_ERR_CUDA;
+    }
+    Dist L = {block_len_mant, block_len_log2};
+    int rc = init_body(st, seed, L, (cudaStream_t)cuda_stream);
+    if (rc) { destroy(st); return rc; }
+    *out = st;
+    return PRAND_OK;
+}
+
+extern "C" int prand_init(prand_state **out, int gen, uint64_t seed, uint64_t n_streams,
+                          uint64_t block_len_mant, unsigned block_len_log2, void *cuda_stream)
+{
+    return prand_init_shard(out, gen, seed, 0, n_streams, block_len_mant, block_len_log2, cuda_stream);
+}
+
+// ==================================================================================================
+// prand_jump (a2)
+// ==================================================================================================
+extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_log2, void *cuda_stream)
+{
+    if (!st) return PRAND_ERR_ARG;
+    if (steps_log2 > 32768) return PRAND_ERR_ARG;
+    if (steps_mant == 0) return PRAND_OK;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    Dist n = {steps_mant, steps_log2};
+    std::vector<unsigned char> ops;
+    int rc = build_level_ops(st->gen, n, 1, ops);
+    if (rc) return rc;
+    rc = ensure_ops(st, ops.size());
+    if (rc) return rc;
+    CU(cudaMemcpyAsync(st->d_ops, ops.data(), ops.size(), cudaMemcpyHostToDevice, stream));
+    LaunchInfo li;
+    if (st->gen == PRAND_MT19937) {
+        uint32_t *d = (uint32_t *)st->d_state[st->cur];
+        CU(mt19937_apply(stream, d, d, 0, st->ns, 0, (const MtOp *)st->d_ops, &li));
+    } else {
+        JumpArgs a;
+        a.base = nullptr;
+        a.st_in = st->d_state[st->cur];
+        a.st_out = st->d_state[st->cur];     // one thread reads and writes its own words only
+        a.n_streams = st->ns;
+        a.ops = st->d_ops;
+        a.idx0 = 1;                          // every stream applies level 0 exactly once
+        a.idx_stride = 0;
+        CU(launch_jump(stream, st->gen, a, &li));
+    }
+    note(st, li);
+    return PRAND_OK;
+}
+
+// ==================================================================================================
+// prand_generate_* (a3-a8)
+// ==================================================================================================
+namespace {
+
+// Launch policy.  With few streams one thread per stream (group) leaves the GPU idle,
+// so a stream's range is cut into sub-sections reached by jump-ahead; outputs are
+// defined by position, so this changes nothing but the schedule.  MT19937 never chunks: applying its
+// jump polynomial costs as much as generating ~10^5 outputs; its kernel is CTA-cooperative instead.
+void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t *chunk_len, uint64_t *n_chunks)
+{
+    *chunk_len = n;
+    *n_chunks = 1;
+    if (gen == PRAND_MT19937 || n == 0) return;
+    uint64_t forced = 0;
+    if (const char *env = std::getenv("PRAND_CHUNK_LEN")) forced = std::strtoull(env, nullptr, 10);
+    uint64_t len;
+    if (forced) {
+        len = forced;
+    } else {
+        // threads one launch gets without chunking
+        uint64_t per_thread_streams = 1, lanes_per_stream = 1, min_len = 64;
+        if (gen == PRAND_LFSR113) per_thread_streams = 4;
+        else if (gen == PRAND_MRG32K3A) per_thread_streams = dtype == DT_F64 ? 2 : 4;
+        else {
+            min_len = 128;
+            if (gen == PRAND_GM61 || gen == PRAND_GQ58_1) lanes_per_stream = 4;
+        }
+        uint64_t threads = ns * lanes_per_stream / per_thread_streams;
+        if (threads == 0) threads = 1;
+        const uint64_t target = (uint64_t)sms * 1024;
+        if (threads >= target) return;
+        uint64_t want = (target + threads - 1) / threads;
+        len = (n + want - 1) / want;
+        if (len < min_len) len = min_len;
+    }
+    len = (len + 3) & ~3ull;                       // the 4-lane GM path stores rows in groups of four
+    if (len >= n) return;
+    *chunk_len = len;
+    *n_chunks = (n + len - 1) / len;
+}
+
+int ensure_chunk_ops(prand_state *st, uint64_t chunk_len, uint64_t n_chunks, cudaStream_t stream)
+{
+    const unsigned levels = bit_length(n_chunks - 1);
+    if (st->d_chunk_ops && st->chunk_len == chunk_len && st->chunk_levels >= levels) return PRAND_OK;
+    std::vector<unsigned char> ops;
+    Dist n = {chunk_len, 0};
+    int rc = build_level_ops(st->gen, n, levels, ops);
+    if (rc) return rc;
+    if (st->d_chunk_ops) { CU(cudaDeviceSynchronize()); CU(cudaFree(st->d_chunk_ops)); st->d_chunk_ops = nullptr; }
+    CU(cudaMalloc(&st->d_chunk_ops, ops.size()));
+    CU(cudaMemcpyAsync(st->d_chunk_ops, ops.data(), ops.size(), cudaMemcpyHostToDevice, stream));
+    st->chunk_len = chunk_len;
+    st->chunk_levels = levels;
+    return PRAND_OK;
+}
+
+int generate(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t stream)
+{
+    if (!st || (!out && n)) return PRAND_ERR_ARG;
+    if (n == 0) return PRAND_OK;
+    const size_t esz = dtype == DT_F64 ? 8 : 4;
+    if ((uintptr_t)out % esz) return PRAND_ERR_ARG;
+    {
+        unsigned __int128 total = (unsigned __int128)n * st->ns * esz;
+        if (total >> 62) return PRAND_ERR_OVERFLOW;
+    }
+    GenArgs a;
+    a.out = out;
+    a.dtype = dtype;
+    a.n_streams = st->ns;
+    a.n = n;
+    plan_chunks(st->gen, st->ns, n, dtype, sm_count(), &a.chunk_len, &a.n_chunks);
+    a.chunk_ops = nullptr;
+    a.st_in = st->d_state[st->cur];
+    a.st_out = st->d_state[st->cur];
+    if (a.n_chunks > 1) {
+        // chunk c reads the start state while the last chunk writes the final one: separate buffers
+        int rc = ensure_second_buffer(st);
+        if (rc) return rc;
+        rc = ensure_chunk_ops(st, a.chunk_len, a.n_chunks, stream);
+        if (rc) return rc;
+        a.chunk_ops = st->d_chunk_ops;
+        a.st_out = st->d_state[1 - st->cur];
+    }
+    LaunchInfo li = {"", 0};
+    cudaError_t e;
+    if (st->gen == PRAND_LFSR113) e = lfsr113_generate(stream, a, &li);
+    else if (st->gen == PRAND_MRG32K3A) e = mrg32k3a_generate(stream, a, &li);
+    else if (st->gen == PRAND_MT19937) e = mt19937_generate(stream, a, &li);
+    else e = gm_generate(stream, st->gen, a, &li);
+    if (e != cudaSuccess) return cuda_fail(e);
+    note(st, li);
+    if (a.n_chunks > 1) st->cur = 1 - st->cur;
+    return PRAND_OK;
+}
+
+// rng_generate_array_: generate on the device in row blocks, copy each block back
+// while the next one is generated.
+int ensure_host_path(prand_state *st, size_t want_bytes)
+{
+    if (!st->host_ready) {
+        CU(cudaStreamCreateWithFlags(&st->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; i++) {
+            CU(cudaEventCreateWithFlags(&st->ev_gen[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&st->ev_copy[i], cudaEventDisableTiming));
+        }
+        st->host_ready = true;
+    }
+    if (st->stage_bytes < want_bytes) {
+        CU(cudaDeviceSynchronize());
+        for (int i = 0; i < 2; i++) {
+            if (st->d_stage[i]) { CU(cudaFree(st->d_stage[i])); st->d_stage[i] = nullptr; }
+            CU(cudaMalloc(&st->d_stage[i], want_bytes));
+        }
+        st->stage_bytes = want_bytes;
+    }
+    return PRAND_OK;
+}
+
+int generate_host(prand_state *st, void *host_out, uint64_t n, int dtype, cudaStream_t stream)
+{
+    if (!st || (!host_out && n)) return PRAND_ERR_ARG;
+    if (n == 0) return PRAND_OK;
+    const size_t esz = dtype == DT_F64 ? 8 : 4;
+    const size_t row_bytes = (size_t)st->ns * esz;
+    const size_t block_target = (size_t)256 << 20;
+    uint64_t rows_per_block = block_target / row_bytes;
+    if (rows_per_block == 0) rows_per_block = 1;
+    if (rows_per_block > n) rows_per_block = n;
+    int rc = ensure_host_path(st, rows_per_block * row_bytes);
+    if (rc) return rc;
+    int slot = 0;
+    uint64_t blocks = 0;
+    for (uint64_t r0 = 0; r0 < n; r0 += rows_per_block, slot ^= 1, blocks++) {
+        const uint64_t rows = n - r0 < rows_per_block ? n - r0 : rows_per_block;
+        if (blocks >= 2) CU(cudaStreamWaitEvent(stream, st->ev_copy[slot], 0));   // slot's previous copy done
+        rc = generate(st, st->d_stage[slot], rows, dtype, stream);
+        if (rc) return rc;
+        CU(cudaEventRecord(st->ev_gen[slot], stream));
+        CU(cudaStreamWaitEvent(st->copy_stream, st->ev_gen[slot], 0));
+        CU(cudaMemcpyAsync((char *)host_out + r0 * row_bytes, st->d_stage[slot], rows * row_bytes,
+                           cudaMemcpyDeviceToHost, st->copy_stream));
+        CU(cudaEventRecord(st->ev_copy[slot], st->copy_stream));
+    }
+    CU(cudaStreamSynchronize(st->copy_stream));
+    CU(cudaStreamSynchronize(stream));
+    return PRAND_OK;
+}
+
+}  // namespace
+
+extern "C" int prand_generate_u32(prand_state *st, uint32_t *out, uint64_t n, void *s)
+{
+    return generate(st, out, n, DT_U32, (cudaStream_t)s);
+}
+extern "C" int prand_generate_f32(prand_state *st, float *out, uint64_t n, void *s)
+{
+    return generate(st, out, n, DT_F32, (cudaStream_t)s);
+}
+extern "C" int prand_generate_f64(prand_state *st, double *out, uint64_t n, void *s)
+{
+    return generate(st, out, n, DT_F64, (cudaStream_t)s);
+}
+extern "C" int prand_generate_u32_host(prand_state *st, uint32_t *out, uint64_t n, void *s)
+{
+    return generate_host(st, out, n, DT_U32, (cudaStream_t)s);
+}
+extern "C" int prand_generate_f32_host(prand_state *st, float *out, uint64_t n, void *s)
+{
+    return generate_host(st, out, n, DT_F32, (cudaStream_t)s);
+}
+extern "C" int prand_generate_f64_host(prand_state *st, double *out, uint64_t n, void *s)
+{
+    return generate_host(st, out, n, DT_F64, (cudaStream_t)s);
+}
+
+// ==================================================================================================
+// canonical state export / import
+// ==================================================================================================
+namespace {
+
+// internal word (w, s) lives at index w * ns + s (SoA) except MT19937, which is [s][624] already
+template <class W> void soa_to_canon(const W *soa, W *canon, uint64_t ns, size_t words)
+{
+    for (size_t w = 0; w < words; w++)
+        for (uint64_t s = 0; s < ns; s++) canon[s * words + w] = soa[w * ns + s];
+}
+template <class W> void canon_to_soa(const W *canon, W *soa, uint64_t ns, size_t words)
+{
+    for (size_t w = 0; w < words; w++)
+        for (uint64_t s = 0; s < ns; s++) soa[w * ns + s] = canon[s * words + w];
+}
+
+}  // namespace
+
+extern "C" size_t prand_state_bytes(const prand_state *st) { return st ? st->bytes : 0; }
+extern "C" uint64_t prand_n_streams(const prand_state *st) { return st ? st->ns : 0; }
+extern "C" int prand_gen_of(const prand_state *st) { return st ? st->gen : PRAND_ERR_ARG; }
+
+extern "C" int prand_get_state(const prand_state *st, void *host_buf, size_t bytes)
+{
+    if (!st || !host_buf) return PRAND_ERR_ARG;
+    if (bytes != st->bytes) return PRAND_ERR_SIZE;
+    CU(cudaDeviceSynchronize());
+    const size_t words = state_words(st->gen);
+    if (st->gen == PRAND_MT19937) {
+        CU(cudaMemcpy(host_buf, st->d_state[st->cur], bytes, cudaMemcpyDeviceToHost));
+        uint32_t *w = (uint32_t *)host_buf;
+        for (uint64_t s = 0; s < st->ns; s++) w[s * words] &= 0x80000000u;   // reading T2
+        return PRAND_OK;
+    }
+    std::vector<unsigned char> tmp(bytes);
+    CU(cudaMemcpy(tmp.data(), st->d_state[st->cur], bytes, cudaMemcpyDeviceToHost));
+    if (state_word_bytes(st->gen) == 8) soa_to_canon((const uint64_t *)tmp.data(), (uint64_t *)host_buf, st->ns, words);
+    else soa_to_canon((const uint32_t *)tmp.data(), (uint32_t *)host_buf, st->ns, words);
+    if (st->gen == PRAND_LFSR113) {                 // reading L3: only the top p bits are state
+        static const uint32_t mask[4] = {0xFFFFFFFEu, 0xFFFFFFF8u, 0xFFFFFFF0u, 0xFFFFFF80u};
+        uint32_t *w = (uint32_t *)host_buf;
+        for (uint64_t s = 0; s < st->ns; s++)
+            for (int c = 0; c < 4; c++) w[4 * s + c] &= mask[c];
+    }
+    return PRAND_OK;
+}
+
+extern "C" int prand_set_state(prand_state *st, const void *host_buf, size_t bytes)
+{
+    if (!st || !host_buf) return PRAND_ERR_ARG;
+    if (bytes != st->bytes) return PRAND_ERR_SIZE;
+    CU(cudaDeviceSynchronize());
+    const size_t words = state_words(st->gen);
+    if (st->gen == PRAND_MT19937) {
+        CU(cudaMemcpy(st->d_state[st->cur], host_buf, bytes, cudaMemcpyHostToDevice));
+        return PRAND_OK;
+    }
+    std::vector<unsigned char> tmp(bytes);
+    if (state_word_bytes(st->gen) == 8) canon_to_soa((const uint64_t *)host_buf, (uint64_t *)tmp.data(), st->ns, words);
+    else canon_to_soa((const uint32_t *)host_buf, (uint32_t *)tmp.data(), st->ns, words);
+    CU(cudaMemcpy(st->d_state[st->cur], tmp.data(), bytes, cudaMemcpyHostToDevice));
+    return PRAND_OK;
+}
+
+extern "C" int prand_free(prand_state *st)
+{
+    if (!st) return PRAND_ERR_ARG;
+    destroy(st);
+    return PRAND_OK;
+}
+
+// ==================================================================================================
+// probes and bookkeeping
+// ==================================================================================================
+extern "C" int prand_fill_u32(uint32_t *out, uint64_t n_words, uint32_t value, void *cuda_stream)
+{
+    if (!out && n_words) return PRAND_ERR_ARG;
+    if ((uintptr_t)out % 16) return PRAND_ERR_ARG;
+    if (n_words == 0) return PRAND_OK;
+    LaunchInfo li = {"", 0};
+    CU(fill_u32((cudaStream_t)cuda_stream, out, n_words, value, &li));
+    note(nullptr, li);
+    return PRAND_OK;
+}
+
+extern "C" uint64_t prand_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+extern "C" const char *prand_last_kernel(const prand_state *st) { return st ? st->last_kernel : ""; }
+extern "C" int prand_last_cuda_error(void) { return g_last_cuda_error; }
+extern "C" const char *prand_version(void) { return "prand-b200 0.1 (sm_100a)"; }
+
+extern "C" const char *prand_strerror(int code)
+{
+    switch (code) {
+    case PRAND_OK: return "ok";
+    case PRAND_ERR_GEN: return "unknown generator";
+    case PRAND_ERR_ARG: return "invalid argument";
+    case PRAND_ERR_SEED: return "seed not valid for this generator";
+    case PRAND_ERR_OVERFLOW: return "stream index times block length mantissa overflows 64 bits";
+    case PRAND_ERR_CUDA: return "CUDA runtime error";
+    case PRAND_ERR_SIZE: return "byte count does not match prand_state_bytes()";
+    case PRAND_ERR_ALLOC: return "allocation failed";
+    case PRAND_ERR_INTERNAL: return "internal self-check failed";
+    default: return "unknown error code";
+    }
+}
+
+// ==================================================================================================
+// host-only hooks (include/prand_host.h)
+// ==================================================================================================
+extern "C" size_t prand_host_skip_op_bytes(int gen)
+{
+    if (gen == PRAND_LFSR113) return sizeof(LfsrOp);
+    if (gen == PRAND_MRG32K3A) return sizeof(MrgOp);
+    if (gen == PRAND_MT19937) return sizeof(MtOp);
+    if (is_gm(gen)) return sizeof(GmOp);
+    return 0;
+}
+
+extern "C" int prand_host_skip_op(int gen, uint64_t mant, unsigned log2, void *buf, size_t bytes)
+{
+    if (gen < 0 || gen >= PRAND_NGEN) return PRAND_ERR_GEN;
+    if (!buf) return PRAND_ERR_ARG;
+    if (bytes != prand_host_skip_op_bytes(gen)) return PRAND_ERR_SIZE;
+    std::vector<unsigned char> ops;
+    Dist n = {mant, log2};
+    int rc = build_level_ops(gen, n, 1, ops);
+    if (rc) return rc;
+    std::memcpy(buf, ops.data(), bytes);
+    return PRAND_OK;
+}
+
+extern "C" size_t prand_host_state_bytes(int gen) { return (gen < 0 || gen >= PRAND_NGEN) ? 0 : stream_bytes(gen); }
+
+extern "C" int prand_host_seed_state(int gen, uint64_t seed, void *buf, size_t bytes)
+{
+    if (gen < 0 || gen >= PRAND_NGEN) return PRAND_ERR_GEN;
+    if (!buf) return PRAND_ERR_ARG;
+    if (bytes != stream_bytes(gen)) return PRAND_ERR_SIZE;
+    std::vector<unsigned char> st;
+    int rc = build_seed_state(gen, seed, st);
+    if (rc) return rc;
+    std::memcpy(buf, st.data(), bytes);
+    return PRAND_OK;
+}
+
+extern "C" int prand_host_mt19937_phi(uint32_t *words624)
+{
+    if (!words624) return PRAND_ERR_ARG;
+    MtOp op;
+    host::mt19937_to_op(host::mt19937_phi(), op);
+    std::memcpy(words624, op.w, sizeof op.w);
+    return PRAND_OK;
+}
+
+extern "C" int prand_host_mt19937_mulmod(const uint32_t *a624, const uint32_t *b624, uint32_t *r624)
+{
+    if (!a624 || !b624 || !r624) return PRAND_ERR_ARG;
+    host::MtPoly a, b, r;
+    std::memcpy(a.w, a624, sizeof a.w);            // little-endian: two u32 words per u64 word
+    std::memcpy(b.w, b624, sizeof b.w);
+    host::mt19937_mulmod(r, a, b);
+    std::memcpy(r624, r.w, sizeof r.w);
+    return PRAND_OK;
+}
+
+extern "C" int prand_host_plan(int gen, uint64_t n_streams, uint64_t n_per_stream, int dtype, int sms,
+                               uint64_t *chunk_len, uint64_t *n_chunks)
+{
+    if (gen < 0 || gen >= PRAND_NGEN) return PRAND_ERR_GEN;
+    if (!chunk_len || !n_chunks || n_streams == 0 || dtype < 0 || dtype > 2 || sms <= 0) return PRAND_ERR_ARG;
+    plan_chunks(gen, n_streams, n_per_stream, dtype, sms, chunk_len, n_chunks);
+    return PRAND_OK;
+}

@@ -1,0 +1,166 @@
+"""CPU tests of libprand's host side (no GPU, no compute call).
+
+  * the library loads and exports every function include/prand.h and include/prand_host.h declare;
+  * step a0 -- the skip operators the host prepares -- applied here to
+    a state with plain Python integers reaches the state the oracle's own jump reaches;
+  * the seed states the host prepares equal the oracle's;
+  * the MT19937 characteristic polynomial from the closed form of ref. [2] equals the oracle's
+    Berlekamp-Massey result, and the polynomial product composes jumps;
+  * the launch policy covers every row exactly once;
+  * argument errors are reported without touching CUDA.
+"""
+import ctypes as C
+import os
+import random
+import re
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1307_5869_b200 as P
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+DISTS = [0, 1, 2, 3, 777, 2**20 + 1, 2**40, 3 * 2**64, 12345 << 76, (2**63 + 5) << 100]
+GM = ["gm19", "gm29", "gm31", "gm55", "gm61", "gq58.1", "gq58.3", "gq58.4"]
+GM_G = {"gm19": 2**19 - 1, "gm29": 2**29 - 3, "gm31": 2**31 - 1, "gm55": 16 * (2**51 - 129),
+        "gm61": 2**61 - 1, "gq58.1": 2**29 * (2**29 - 3), "gq58.3": 2**29 * (2**29 - 3),
+        "gq58.4": 2**29 * (2**29 - 3)}
+M1, M2 = 2**32 - 209, 2**32 - 22853
+LFSR_MASK = [0xFFFFFFFE, 0xFFFFFFF8, 0xFFFFFFF0, 0xFFFFFF80]
+
+
+def declared_functions():
+    names = []
+    for hdr in ("prand.h", "prand_host.h"):
+        text = open(os.path.join(ROOT, "include", hdr)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names += re.findall(r"\b(prand_[a-z0-9_]+)\s*\(", text)
+    return sorted(set(names))
+
+
+def test_library_exports_every_declared_symbol():
+    names = declared_functions()
+    assert len(names) >= 25
+    raw = C.CDLL(P.LIB_PATH)
+    for n in names:
+        assert hasattr(raw, n), f"libprand.so does not export {n}"
+    # and the binding knows each of them
+    assert set(names) == set(P.EXPORTS)
+
+
+def test_version_and_strerror():
+    assert b"sm_100a" in P.lib().prand_version()
+    assert P.lib().prand_strerror(0) == b"ok"
+    for code in range(-8, 0):
+        assert P.lib().prand_strerror(code) not in (b"ok", b"unknown error code")
+
+
+def test_argument_errors_before_any_cuda_call():
+    h = C.c_void_p()
+    L = P.lib()
+    assert L.prand_init(C.byref(h), 99, 1, 1, 1, 0, None) == -1          # bad generator
+    assert L.prand_init(C.byref(h), 0, 12345, 0, 1, 0, None) == -2        # no streams
+    assert L.prand_init(C.byref(h), 0, 100, 4, 1, 0, None) == -3          # LFSR113 seed < 128
+    assert L.prand_init(C.byref(h), 1, 0, 4, 1, 0, None) == -3            # MRG32K3A seed 0
+    assert L.prand_init(C.byref(h), 1, 2**32 - 1, 4, 1, 0, None) == -3    # MRG32K3A seed >= m2
+    assert L.prand_init(C.byref(h), 2, 2**32, 4, 1, 0, None) == -3        # MT19937 seed >= 2^32
+    assert L.prand_init(C.byref(h), 3, 2**19 - 1, 4, 1, 0, None) == -3    # GM19 seed = 0 mod g
+    assert L.prand_init(C.byref(h), 0, 12345, 2**40, 2**40, 0, None) == -4  # s * mant overflows
+    assert L.prand_init(None, 0, 12345, 4, 1, 0, None) == -2
+    assert h.value is None
+    assert L.prand_generate_u32(None, None, 4, None) == -2
+    assert L.prand_jump(None, 1, 0, None) == -2
+    assert L.prand_free(None) == -2
+
+
+@pytest.mark.parametrize("dist", DISTS)
+def test_lfsr113_skip_operator_reaches_oracle_state(dist):
+    op = np.frombuffer(P.prand_host_skip_op("lfsr113", dist), dtype=np.uint32).reshape(4, 32)
+    for seed in (12345, 0xDEADBEEF):
+        z = np.frombuffer(P.prand_host_seed_state("lfsr113", seed), dtype=np.uint32)
+        got = []
+        for c in range(4):
+            r = 0
+            for j in range(32):
+                if (int(z[c]) >> j) & 1:
+                    r ^= int(op[c, j])
+            got.append(r & LFSR_MASK[c])
+        want = np.frombuffer(oracle.State("lfsr113", seed).jump(dist).export(), dtype=np.uint32)
+        assert got == want.tolist()
+
+
+@pytest.mark.parametrize("dist", DISTS)
+def test_mrg32k3a_skip_operator_reaches_oracle_state(dist):
+    op = np.frombuffer(P.prand_host_skip_op("mrg32k3a", dist), dtype=np.uint32).astype(object)
+    A, B = op[:9].reshape(3, 3), op[9:].reshape(3, 3)
+    st = np.frombuffer(P.prand_host_seed_state("mrg32k3a", 12345), dtype=np.uint32).astype(object)
+    x = [sum(A[i, j] * st[j] for j in range(3)) % M1 for i in range(3)]
+    y = [sum(B[i, j] * st[3 + j] for j in range(3)) % M2 for i in range(3)]
+    want = np.frombuffer(oracle.State("mrg32k3a", 12345).jump(dist).export(), dtype=np.uint32)
+    assert x + y == want.tolist()
+
+
+@pytest.mark.parametrize("gen", GM)
+def test_gm_skip_operator_and_seed_state_reach_oracle_state(gen):
+    g = GM_G[gen]
+    dt = np.uint32 if g < 2**32 else np.uint64
+    for seed in (1, 987654321987):
+        if seed % g == 0:
+            continue
+        base = np.frombuffer(P.prand_host_seed_state(gen, seed), dtype=dt).astype(object)
+        assert base.tolist() == np.frombuffer(oracle.State(gen, seed).export(), dtype=dt).tolist()
+        for dist in DISTS:
+            m = np.frombuffer(P.prand_host_skip_op(gen, dist), dtype=np.uint64).astype(object)
+            got = []
+            for i in range(len(base) // 2):
+                xP, xN = base[2 * i], base[2 * i + 1]
+                got += [(m[2] * xN + m[3] * xP) % g, (m[0] * xN + m[1] * xP) % g]
+            want = np.frombuffer(oracle.State(gen, seed).jump(dist).export(), dtype=dt).tolist()
+            assert got == want, (gen, seed, dist)
+
+
+def test_mt19937_phi_closed_form_equals_oracle_minimal_polynomial():
+    deg, phi = oracle.mt19937_charpoly()
+    mine = np.frombuffer(P.prand_host_mt19937_phi(), dtype=np.uint64)
+    assert deg == 19937
+    assert np.array_equal(mine[:312], phi)
+    assert sum(bin(int(w)).count("1") for w in mine) == 135     # 135 non-zero terms
+
+
+@pytest.mark.parametrize("dist", [0, 1, 5, 623, 624, 19937, 50000, 2**64, (2**40 + 5) << 64, 12345 << 3])
+def test_mt19937_jump_polynomial_equals_oracle(dist):
+    a = np.frombuffer(P.prand_host_skip_op("mt19937", dist), dtype=np.uint64)
+    assert np.array_equal(a, oracle.mt19937_jump_poly(dist))
+
+
+def test_mt19937_polynomial_product_composes_jumps():
+    rng = random.Random(7)
+    for _ in range(4):
+        a, b = rng.randrange(1, 2**60), rng.randrange(1, 2**60) << rng.randrange(0, 80)
+        pa, pb = P.prand_host_skip_op("mt19937", a), P.prand_host_skip_op("mt19937", b)
+        prod = np.frombuffer(P.prand_host_mt19937_mulmod(pa, pb), dtype=np.uint64)
+        assert np.array_equal(prod, oracle.mt19937_jump_poly(a + b))
+
+
+def test_mt19937_seed_state_equals_oracle():
+    mine = np.frombuffer(P.prand_host_seed_state("mt19937", 5489), dtype=np.uint32).copy()
+    want = np.frombuffer(oracle.State("mt19937", 5489).export(), dtype=np.uint32)
+    mine[0] &= 0x80000000
+    assert np.array_equal(mine, want)
+
+
+@pytest.mark.parametrize("gen", ["lfsr113", "mrg32k3a", "gm31", "gm61", "gq58.3", "mt19937"])
+def test_plan_covers_all_rows(gen):
+    for ns in (1, 5, 512, 1024, 65536, 2**20):
+        for n in (1, 3, 64, 100, 4096, 2**20):
+            for dt in ("u32", "f64"):
+                cl, nc = P.prand_host_plan(gen, ns, n, dt, 148)
+                assert nc >= 1 and cl >= 1
+                assert (nc - 1) * cl < n <= nc * cl
+                if nc > 1:
+                    assert cl % 4 == 0 and gen != "mt19937"
+    # enough streams: never chunk
+    assert P.prand_host_plan("lfsr113", 2**20, 2048, "u32", 148) == (2048, 1)
+    # config 1 (1024 streams x 4096) must be cut to fill the GPU
+    assert P.prand_host_plan("lfsr113", 1024, 4096, "u32", 148)[1] > 1
