@@ -1,0 +1,104 @@
+"""GPU parity at BASELINE.json's full sizes (configs C1..C5), in the launch configuration bench.py times.
+
+The oracle cannot produce 2^30 numbers in seconds, but every stream is defined by position
+(stream s = base sequence advanced s * block_len), so it can compute any single
+stream on its own: each test generates the whole configuration on the GPU and compares ALL rows of a
+sample of streams (first, last, around CTA / warp boundaries, seeded random ones) plus the exported
+final states of those streams, bit for bit.  C1 is small enough to compare completely.
+"""
+import os
+import random
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+import paper_1307_5869_b200 as P  # noqa: E402
+
+NPDT = {"u32": np.uint32, "f32": np.float32, "f64": np.float64}
+BITS = {"u32": np.uint32, "f32": np.uint32, "f64": np.uint64}
+TDT = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}
+CPU_THREADS = min(16, os.cpu_count() or 1)
+
+
+def need_gpu(min_free_bytes=0):
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    free, _ = torch.cuda.mem_get_info()
+    if free < min_free_bytes:
+        pytest.skip(f"needs {min_free_bytes >> 30} GiB of free device memory")
+
+
+def sample_streams(ns, k, seed):
+    """Boundary streams (CTA / warp / vector-group edges) plus seeded random ones, at least k."""
+    fixed = [0, 1, 3, 4, 31, 32, 127, 128, 255, 256, ns // 2 - 1, ns // 2, ns - 129, ns - 33, ns - 2, ns - 1]
+    rng = random.Random(seed)
+    picks = {s for s in fixed if 0 <= s < ns}
+    while len(picks) < min(k, ns):
+        picks.add(rng.randrange(ns))
+    return sorted(picks)
+
+
+def check_config(w, n_sample):
+    state_bytes = w.n_streams * oracle.state_bytes(w.gen)
+    need_gpu(w.out_bytes + 3 * state_bytes + (1 << 30))
+    g = P.Generator(w.gen, w.seed, w.n_streams, w.block_len)
+    out = torch.empty((w.n_per_stream, w.n_streams), dtype=TDT[w.dtype], device="cuda")
+    g.generate(w.n_per_stream, w.dtype, out=out)
+    torch.cuda.synchronize()
+    picks = sample_streams(w.n_streams, n_sample, seed=w.n_streams ^ w.n_per_stream)
+    idx = torch.tensor(picks, device="cuda")
+    got = out.index_select(1, idx).cpu().numpy().view(NPDT[w.dtype])
+    del out
+    sb = oracle.state_bytes(w.gen)
+    states = g.state() if state_bytes <= (1 << 30) else None
+    kernel = g.last_kernel
+    g.close()
+    torch.cuda.empty_cache()
+    for j, s in enumerate(picks):
+        want, wst = oracle.streams(w.gen, w.seed, s, 1, w.block_len, w.n_per_stream, w.dtype)
+        gb = np.ascontiguousarray(got[:, j]).view(BITS[w.dtype])
+        wb = np.ascontiguousarray(want[:, 0]).view(BITS[w.dtype])
+        if not np.array_equal(gb, wb):
+            i = int(np.argmax(gb != wb))
+            raise AssertionError(f"{w.name} [{kernel}] stream {s}: {(gb != wb).sum()} of {len(gb)} differ; first at "
+                                 f"row {i}: got {got[i, j]!r} want {want[i, 0]!r}")
+        if states is not None:
+            assert states[s * sb:(s + 1) * sb] == wst.tobytes(), f"{w.name} stream {s}: final state differs"
+
+
+def test_c1_lfsr113_complete():
+    w = workloads.C1
+    need_gpu()
+    g = P.Generator(w.gen, w.seed, w.n_streams, w.block_len)
+    got = g.generate(w.n_per_stream, w.dtype).cpu().numpy().view(np.uint32)
+    st = g.state()
+    assert "lfsr113" in g.last_kernel
+    g.close()
+    want, wst = oracle.streams(w.gen, w.seed, 0, w.n_streams, w.block_len, w.n_per_stream, w.dtype,
+                               threads=CPU_THREADS)
+    assert np.array_equal(got, want)
+    assert st == wst.tobytes()
+
+
+def test_c2_mrg32k3a_f64_full_size_sampled():
+    check_config(workloads.C2, 48)
+
+
+def test_c3_mt19937_full_size_sampled():
+    check_config(workloads.C3, 6)          # each sampled stream costs the oracle a 2^64-scale polynomial
+
+
+@pytest.mark.parametrize("w", workloads.C4, ids=lambda w: w.name)
+def test_c4_gm_f32_full_size_sampled(w):
+    check_config(w, 24)
+
+
+@pytest.mark.parametrize("w", workloads.C5, ids=lambda w: w.name)
+def test_c5_sweep_full_size_sampled(w):
+    check_config(w, 6 if w.gen == "mt19937" else 40)

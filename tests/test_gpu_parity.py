@@ -1,0 +1,216 @@
+"""GPU parity tests: libprand (CUDA, through the C ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): bit-exact for uint32 outputs and exported states; f32/f64 are
+compared bit-exactly too (both sides convert an exactly representable integer with a power-of-two
+scale, or one IEEE multiply for MRG32K3A's f64 -- DESIGN.md "Tolerance"), so the |d| <= 2^-24 / 2^-53
+fallback is never needed.  Small cases compare every output of every stream at sizes that span
+several thread groups / tiles with ragged tails; the BASELINE.json configurations run at full size in
+the launch configuration bench.py times and are compared on sampled streams (all rows of each).
+"""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+from workloads import Workload
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+import paper_1307_5869_b200 as P  # noqa: E402
+
+ALL_GENS = P.GENS
+NPDT = {"u32": np.uint32, "f32": np.float32, "f64": np.float64}
+BITS = {"u32": np.uint32, "f32": np.uint32, "f64": np.uint64}
+CPU_THREADS = min(16, os.cpu_count() or 1)
+
+
+def need_gpu():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+
+
+def as_bits(a: np.ndarray, dtype: str) -> np.ndarray:
+    return np.ascontiguousarray(a).view(BITS[dtype])
+
+
+def lib_run(w: Workload, first=0, pre_jump=0, calls=None):
+    """Generate w on the GPU -> (out as numpy (n, ns), canonical state bytes, kernel name)."""
+    g = P.Generator(w.gen, w.seed, w.n_streams, w.block_len, first_stream=first)
+    if pre_jump:
+        g.jump(pre_jump)
+    parts = []
+    for n in (calls or [w.n_per_stream]):
+        parts.append(g.generate(n, w.dtype))
+    torch.cuda.synchronize()
+    out = torch.cat(parts, 0).cpu().numpy().view(NPDT[w.dtype])
+    st, k = g.state(), g.last_kernel
+    g.close()
+    return out, st, k
+
+
+def oracle_run(w: Workload, first=0, pre_jump=0):
+    out, states = oracle.streams(w.gen, w.seed, first, w.n_streams, w.block_len, w.n_per_stream,
+                                 w.dtype, threads=CPU_THREADS, pre_jump=pre_jump)
+    return out, states.tobytes()
+
+
+def assert_same(w, got, want, what="outputs"):
+    gb, wb = as_bits(got, w.dtype), as_bits(want, w.dtype)
+    if not np.array_equal(gb, wb):
+        bad = np.argwhere(gb != wb)
+        i, s = bad[0]
+        raise AssertionError(f"{w.name} {w.gen}/{w.dtype}: {len(bad)} of {gb.size} {what} differ; first at "
+                             f"row {i} stream {s}: got {got[i, s]!r} want {want[i, s]!r}")
+
+
+def small_cases(gen):
+    # (n_streams, n_per_stream, block_len): a ragged stream count (scalar store path), a count that is
+    # a multiple of 4 but of no CTA size, rows that are no multiple of the unroll / tile height
+    if gen == "mt19937":      # the oracle's per-stream polynomial costs ~1 s at 2^64: keep streams few
+        return [(5, 700, 2**64), (37, 70, 1000), (64, 33, 12345)]
+    return [(37, 53, workloads.BLOCK_LEN[gen]), (1000, 67, workloads.BLOCK_LEN[gen]), (260, 129, 3)]
+
+
+@pytest.mark.parametrize("dtype", ["u32", "f32", "f64"])
+@pytest.mark.parametrize("gen", ALL_GENS)
+def test_every_output_and_state_matches_oracle(gen, dtype):
+    need_gpu()
+    for ns, n, L in small_cases(gen):
+        w = Workload(f"small-{ns}x{n}", gen, workloads.SEED.get(gen, 1), ns, L, n, dtype)
+        got, st, _ = lib_run(w)
+        want, wst = oracle_run(w)
+        assert_same(w, got, want)
+        assert st == wst, f"{w.name} {gen}: exported states differ"
+
+
+@pytest.mark.parametrize("gen", ALL_GENS)
+def test_successive_calls_continue_the_streams(gen):
+    need_gpu()
+    ns, L = (6, 2**64) if gen == "mt19937" else (132, workloads.BLOCK_LEN[gen])
+    w = Workload("continue", gen, workloads.SEED.get(gen, 1), ns, L, 700, "u32")
+    got, st, _ = lib_run(w, calls=[1, 0, 30, 600, 69])
+    want, wst = oracle_run(w)
+    assert_same(w, got, want)
+    assert st == wst
+
+
+@pytest.mark.parametrize("gen", ALL_GENS)
+def test_prand_jump_advances_every_stream(gen):
+    need_gpu()
+    ns, L = (4, 2**64) if gen == "mt19937" else (68, workloads.BLOCK_LEN[gen])
+    for steps in (1, 1000, 5 << 70):
+        if gen == "gm19" and steps > 2**30:
+            continue
+        w = Workload("jump", gen, workloads.SEED.get(gen, 1), ns, L, 40, "u32")
+        got, st, _ = lib_run(w, pre_jump=steps)
+        want, wst = oracle_run(w, pre_jump=steps)
+        assert_same(w, got, want)
+        assert st == wst
+
+
+@pytest.mark.parametrize("gen", [g for g in ALL_GENS if g != "mt19937"])
+def test_sub_section_chunking_changes_nothing(gen, monkeypatch):
+    """a stream's range cut into sections reached by jump-ahead yields the same numbers."""
+    need_gpu()
+    w = Workload("chunked", gen, workloads.SEED.get(gen, 1), 44, workloads.BLOCK_LEN[gen], 203, "f32")
+    want, wst = oracle_run(w)
+    for chunk in (4, 8, 52, 200):
+        monkeypatch.setenv("PRAND_CHUNK_LEN", str(chunk))
+        got, st, _ = lib_run(w, calls=[150, 53])
+        assert_same(w, got, want)
+        assert st == wst
+    monkeypatch.delenv("PRAND_CHUNK_LEN")
+
+
+@pytest.mark.parametrize("gen", ["lfsr113", "mrg32k3a", "mt19937", "gm29", "gm61", "gq58.3"])
+def test_shard_holds_its_slice_of_the_global_family(gen):
+    need_gpu()
+    L = 2**64 if gen == "mt19937" else workloads.BLOCK_LEN[gen]
+    first, ns = (5, 7) if gen == "mt19937" else (1029, 75)
+    w = Workload("shard", gen, workloads.SEED.get(gen, 1), ns, L, 31, "u32")
+    got, st, _ = lib_run(w, first=first)
+    want, wst = oracle_run(w, first=first)
+    assert_same(w, got, want)
+    assert st == wst
+
+
+@pytest.mark.parametrize("gen", ALL_GENS)
+def test_state_roundtrip_through_the_host(gen):
+    """the state is plain data; copied out and back in, generation continues from it."""
+    need_gpu()
+    ns, L = (3, 1000) if gen == "mt19937" else (21, workloads.BLOCK_LEN[gen])
+    seed = workloads.SEED.get(gen, 1)
+    a = P.Generator(gen, seed, ns, L)
+    a.generate(77, "u32")
+    blob = a.state()
+    rest_a = a.generate(50, "u32").cpu().numpy()
+    b = P.Generator(gen, seed, ns, 0)            # block_len 0: all streams identical, then overwritten
+    b.set_state(blob)
+    assert b.state() == blob
+    rest_b = b.generate(50, "u32").cpu().numpy()
+    assert np.array_equal(rest_a, rest_b)
+    want, _ = oracle.streams(gen, seed, 0, ns, L, 127, "u32", threads=CPU_THREADS)
+    assert np.array_equal(rest_a.view(np.uint32), want[77:])
+    a.close(); b.close()
+
+
+@pytest.mark.parametrize("gen,dtype", [("lfsr113", "u32"), ("mrg32k3a", "f64"), ("gm31", "f32"), ("mt19937", "u32")])
+def test_host_delivery_equals_device_fill(gen, dtype):
+    """rng_generate_array_: same numbers, delivered to host memory."""
+    need_gpu()
+    ns, L = (6, 1000) if gen == "mt19937" else (300, workloads.BLOCK_LEN[gen])
+    w = Workload("host", gen, workloads.SEED.get(gen, 1), ns, L, 90, dtype)
+    want, _ = oracle_run(w)
+    g = P.Generator(w.gen, w.seed, w.n_streams, w.block_len)
+    got = g.generate_host(w.n_per_stream, dtype).numpy().view(NPDT[dtype])
+    assert_same(w, got, want)
+    pageable = torch.empty((w.n_per_stream, ns), dtype=got_dtype(dtype))
+    g2 = P.Generator(w.gen, w.seed, w.n_streams, w.block_len)
+    g2.generate_host(w.n_per_stream, dtype, out=pageable)
+    assert_same(w, pageable.numpy().view(NPDT[dtype]), want)
+    g.close(); g2.close()
+
+
+def got_dtype(dtype):
+    return {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
+
+
+def test_degenerate_sizes_and_errors():
+    need_gpu()
+    g = P.Generator("lfsr113", 12345, 1, 2**40)
+    out = g.generate(1, "u32")
+    assert int(out.view(torch.int32)[0, 0]) & 0xFFFFFFFF == 3338197162   # SURVEY.md 8(c) sample value
+    g.generate(0, "u32")                                                   # no-op
+    assert P.lib().prand_generate_u32(g._h, None, 5, None) == -2
+    buf = torch.empty(8, dtype=torch.int32, device="cuda")
+    assert P.lib().prand_generate_f64(g._h, buf.data_ptr() + 4, 1, None) == -2   # misaligned for f64
+    assert P.lib().prand_get_state(g._h, buf.data_ptr(), 3) == -6
+    g.close()
+    # block_len 0: every stream is the base sequence
+    g = P.Generator("mrg32k3a", 12345, 9, 0)
+    o = g.generate(4, "u32").cpu().numpy()
+    assert (o == o[:, :1]).all()
+    g.close()
+
+
+def test_fill_probe_writes_every_word():
+    need_gpu()
+    for n in (1, 4, 1023, 4096 + 3, 1 << 22):
+        buf = torch.zeros(n + 4, dtype=torch.int32, device="cuda")
+        P.prand_fill_u32(buf.data_ptr(), n, 0x5A5A5A5A)
+        torch.cuda.synchronize()
+        h = buf.cpu().numpy().view(np.uint32)
+        assert (h[:n] == 0x5A5A5A5A).all() and (h[n:] == 0).all()
+
+
+def test_launch_counter_counts_kernels():
+    need_gpu()
+    before = P.prand_launch_count()
+    g = P.Generator("gm55", 1, 64, 2**33)
+    g.generate(8, "u32"); g.generate(8, "f32")
+    assert P.prand_launch_count() - before == 3          # init + two fills
+    assert "gm55" in g.last_kernel
+    g.close()
