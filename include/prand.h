@@ -152,6 +152,9 @@ int prand_fill_u32(uint32_t *out, uint64_t n_words, uint32_t value, void *cuda_s
 /* Number of kernels this library has launched in this process (for bench.py's gpu_launches). */
 uint64_t prand_launch_count(void);
 
+/* Bytes of prepared operator tables / seed states this library has copied host-to-device so far. */
+uint64_t prand_uploaded_bytes(void);
+
 /* Name of the kernel configuration the last generate call on `st` used (static string). */
 const char *prand_last_kernel(const prand_state *st);
 

@@ -40,6 +40,7 @@ _SIGS = {
     "prand_free": (C.c_int, [C.c_void_p]),
     "prand_fill_u32": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p]),
     "prand_launch_count": (C.c_uint64, []),
+    "prand_uploaded_bytes": (C.c_uint64, []),
     "prand_last_kernel": (C.c_char_p, [C.c_void_p]),
     "prand_strerror": (C.c_char_p, [C.c_int]),
     "prand_last_cuda_error": (C.c_int, []),
@@ -179,6 +180,10 @@ def prand_fill_u32(out_ptr: int, n_words: int, value: int, stream=None) -> None:
 
 def prand_launch_count() -> int:
     return lib().prand_launch_count()
+
+
+def prand_uploaded_bytes() -> int:
+    return lib().prand_uploaded_bytes()
 
 
 def prand_last_kernel(state: int) -> str:

@@ -63,6 +63,7 @@ int sm_count()
 namespace {
 
 std::atomic<uint64_t> g_launches{0};
+std::atomic<uint64_t> g_h2d_bytes{0};   // operator tables and seed states uploaded by init/jump/generate
 thread_local int g_last_cuda_error = 0;
 
 inline bool is_gm(int gen) { return gen >= PRAND_GM19 && gen <= PRAND_GQ58_4; }
@@ -90,6 +91,12 @@ int cuda_fail(cudaError_t e)
     g_last_cuda_error = (int)e;
     return PRAND_ERR_CUDA;
 }
+// host-to-device upload of a prepared table, counted for bench.py's h2d_bytes_per_step
+#define UPLOAD(dst, src, bytes, stream)                                                        \
+    do {                                                                                       \
+        CU(cudaMemcpyAsync((dst), (src), (bytes), cudaMemcpyHostToDevice, (stream)));          \
+        g_h2d_bytes.fetch_add((bytes), std::memory_order_relaxed);                             \
+    } while (0)
 #define CU(call)                                         \
     do {                                                 \
         cudaError_t e_ = (call);                         \
@@ -238,9 +245,9 @@ int init_mt19937(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
     }
     rc = ensure_ops(st, ops.size() * sizeof(MtOp));
     if (rc) return rc;
-    CU(cudaMemcpyAsync(st->d_ops, ops.data(), ops.size() * sizeof(MtOp), cudaMemcpyHostToDevice, stream));
+    UPLOAD(st->d_ops, ops.data(), ops.size() * sizeof(MtOp), stream);
     uint32_t *d = (uint32_t *)st->d_state[st->cur];
-    CU(cudaMemcpyAsync(d, base.data(), base.size(), cudaMemcpyHostToDevice, stream));
+    UPLOAD(d, base.data(), base.size(), stream);
     const MtOp *d_ops = (const MtOp *)st->d_ops;
     LaunchInfo li;
     if (have_first) {
@@ -268,9 +275,9 @@ int init_body(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
     const size_t ops_off = (base.size() + 255) & ~(size_t)255;
     rc = ensure_ops(st, ops_off + ops.size() + 256);
     if (rc) return rc;
-    CU(cudaMemcpyAsync(st->d_ops, base.data(), base.size(), cudaMemcpyHostToDevice, stream));
+    UPLOAD(st->d_ops, base.data(), base.size(), stream);
     if (!ops.empty())
-        CU(cudaMemcpyAsync((char *)st->d_ops + ops_off, ops.data(), ops.size(), cudaMemcpyHostToDevice, stream));
+        UPLOAD((char *)st->d_ops + ops_off, ops.data(), ops.size(), stream);
     JumpArgs a;
     a.base = st->d_ops;
     a.st_in = nullptr;
@@ -365,7 +372,7 @@ extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_l
     if (rc) return rc;
     rc = ensure_ops(st, ops.size());
     if (rc) return rc;
-    CU(cudaMemcpyAsync(st->d_ops, ops.data(), ops.size(), cudaMemcpyHostToDevice, stream));
+    UPLOAD(st->d_ops, ops.data(), ops.size(), stream);
     LaunchInfo li;
     if (st->gen == PRAND_MT19937) {
         uint32_t *d = (uint32_t *)st->d_state[st->cur];
@@ -437,7 +444,7 @@ int ensure_chunk_ops(prand_state *st, uint64_t chunk_len, uint64_t n_chunks, cud
     if (rc) return rc;
     if (st->d_chunk_ops) { CU(cudaDeviceSynchronize()); CU(cudaFree(st->d_chunk_ops)); st->d_chunk_ops = nullptr; }
     CU(cudaMalloc(&st->d_chunk_ops, ops.size()));
-    CU(cudaMemcpyAsync(st->d_chunk_ops, ops.data(), ops.size(), cudaMemcpyHostToDevice, stream));
+    UPLOAD(st->d_chunk_ops, ops.data(), ops.size(), stream);
     st->chunk_len = chunk_len;
     st->chunk_levels = levels;
     return PRAND_OK;
@@ -650,6 +657,7 @@ extern "C" int prand_fill_u32(uint32_t *out, uint64_t n_words, uint32_t value, v
 }
 
 extern "C" uint64_t prand_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+extern "C" uint64_t prand_uploaded_bytes(void) { return g_h2d_bytes.load(std::memory_order_relaxed); }
 extern "C" const char *prand_last_kernel(const prand_state *st) { return st ? st->last_kernel : ""; }
 extern "C" int prand_last_cuda_error(void) { return g_last_cuda_error; }
 extern "C" const char *prand_version(void) { return "prand-b200 0.1 (sm_100a)"; }
