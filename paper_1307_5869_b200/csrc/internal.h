@@ -45,8 +45,9 @@ struct JumpArgs {
 };
 
 // One bulk generation launch.  Rows [0, n) of every stream; when n_chunks > 1 virtual stream
-// (s, c) first jumps c * chunk_len ahead with chunk_ops (levels = bits of c) and fills rows
-// [c*chunk_len, min(n, (c+1)*chunk_len)); the last chunk writes the final state to st_out.
+// (s, c) first jumps c * chunk_len ahead with chunk_ops[c - 1] (the operator of distance
+// c * chunk_len, c = 1..n_chunks-1) and fills rows [c*chunk_len, min(n, (c+1)*chunk_len)); the last
+// chunk writes the final state to st_out.
 struct GenArgs {
     const void *st_in;
     void *st_out;

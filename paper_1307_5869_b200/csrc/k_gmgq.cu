@@ -229,7 +229,7 @@ gm_gen_kernel(const typename Gm<GEN>::W *st_in, typename Gm<GEN>::W *st_out,
 #pragma unroll
         for (int j = 0; j < PPL; j++) {
             uint64_t a = xP[j], b = xN[j];
-            gm_apply_bits(chunk_ops, c, a, b, B);
+            gm_apply_bits(chunk_ops + (c - 1), 1, a, b, B);   // operator of c * chunk_len
             xP[j] = (W)a; xN[j] = (W)b;
         }
     }

@@ -86,7 +86,7 @@ lfsr113_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
     }
     if (c != 0) {
 #pragma unroll
-        for (int v = 0; v < V; v++) lfsr113_apply_bits(chunk_ops, c, z[v]);
+        for (int v = 0; v < V; v++) lfsr113_apply_bits(chunk_ops + (c - 1), 1, z[v]);   // operator of c * chunk_len
     }
     const uint64_t row0 = c * chunk_len;
     const uint64_t row1 = (row0 + chunk_len < n) ? row0 + chunk_len : n;

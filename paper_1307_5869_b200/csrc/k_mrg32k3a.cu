@@ -15,42 +15,45 @@ namespace {
 constexpr uint32_t M1 = 4294967087u, M2 = 4294944443u;
 constexpr uint32_t C1 = 209u, C2 = 22853u;
 
-// t < 2^54  ->  t mod m1
-__device__ __forceinline__ uint32_t reduce_m1(uint64_t t)
-{
-    uint64_t u = (uint64_t)(uint32_t)(t >> 32) * C1 + (uint32_t)t;   // < 2^22*209 + 2^32 < 2^32 + 2^30
-    uint32_t lo = (uint32_t)u;
-    uint32_t r = lo + (uint32_t)(u >> 32) * C1;                      // hi in {0,1}; no wrap when hi = 1
-    return r >= M1 ? r - M1 : r;
-}
-// t < 2^54  ->  t mod m2
-__device__ __forceinline__ uint32_t reduce_m2(uint64_t t)
-{
-    uint64_t u = (uint64_t)(uint32_t)(t >> 32) * C2 + (uint32_t)t;   // < 2^22*22853 + 2^32 < 2^37
-    uint64_t w = (uint64_t)(uint32_t)(u >> 32) * C2 + (uint32_t)u;   // < 2^5*22853 + 2^32 < 2 m2
-    return (uint32_t)(w >= M2 ? w - M2 : w);
-}
-
 struct Mrg { uint32_t x0, x1, x2, y0, y1, y2; };   // x0 = x_n, x1 = x_{n-1}, x2 = x_{n-2}
 
-__device__ __forceinline__ uint32_t mrg_step(Mrg &s)
+// x_{n+1} = (a x_{n-1} - b x_{n-2}) mod m1 from (x_{n-1}, x_{n-2}).  t = a x1 + b (m1 - x2) < 2^54,
+// t = hi 2^32 + lo; with the quotient estimate hi + 1:  t - (hi+1) m1 = lo + (hi+1) 209 - 2^32.
+// If the 32-bit addition carries the difference is the wrapped sum (< 2^30 < m1); otherwise the
+// estimate was one too large and adding m1 back gives sum - 209 in [0, m1).  Either way canonical.
+__device__ __forceinline__ uint32_t mrg_next_x(uint32_t x1, uint32_t x2, uint32_t c1)
 {
-    uint64_t tx = (uint64_t)1403580u * s.x1 + (uint64_t)810728u * (M1 - s.x2);
-    uint64_t ty = (uint64_t)527612u * s.y0 + (uint64_t)1370589u * (M2 - s.y2);
-    uint32_t nx = reduce_m1(tx), ny = reduce_m2(ty);
-    s.x2 = s.x1; s.x1 = s.x0; s.x0 = nx;
-    s.y2 = s.y1; s.y1 = s.y0; s.y0 = ny;
-    // z = (x - y) mod m1 with x < m1, y < m2 (y may be >= m1 by at most m2 - m1 < m1)
-    uint32_t yy = ny >= M1 ? ny - M1 : ny;
-    return nx >= yy ? nx - yy : nx + (M1 - yy);
+    uint64_t t = (uint64_t)1403580u * x1 + (uint64_t)810728u * (M1 - x2);
+    uint32_t p = (uint32_t)(t >> 32) * c1 + c1;          // (hi + 1) * 209 < 2^30
+    uint32_t s = (uint32_t)t + p;
+    return s >= p ? s - C1 : s;                          // s >= p  <=>  no carry
+}
+// y_{n+1} = (c y_n - d y_{n-2}) mod m2 from (y_n, y_{n-2}).  One 64-bit fold u = hi 22853 + lo
+// (< 2^38, same residue; the carry chain keeps it out of a register pair), then the same
+// estimate-and-correct step on u = uh 2^32 + ul.
+__device__ __forceinline__ uint32_t mrg_next_y(uint32_t y0, uint32_t y2)
+{
+    uint64_t t = (uint64_t)527612u * y0 + (uint64_t)1370589u * (M2 - y2);
+    uint64_t f = (uint64_t)(uint32_t)(t >> 32) * C2;     // u = f + lo(t), kept as (uh + 1, ul)
+    uint32_t ul, uh1;
+    asm("add.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %4, 1;"
+        : "=r"(ul), "=r"(uh1) : "r"((uint32_t)f), "r"((uint32_t)t), "r"((uint32_t)(f >> 32)));
+    uint32_t p = uh1 * C2;                               // (uh + 1) * 22853 < 2^21
+    uint32_t s = ul + p;
+    return s >= p ? s - C2 : s;
 }
 
-template <int DT> __device__ __forceinline__ typename OutElem<DT>::type mrg_convert(uint32_t z)
+// Output of the combined generator from canonical x < m1, y < m2 < m1 (reading M1):
+// z = (x - y) mod m1 in [0, m1); the f64 map sends z = 0 to m1 (reading M3), i.e. z in [1, m1].
+template <int DT> __device__ __forceinline__ typename OutElem<DT>::type mrg_output(uint32_t x, uint32_t y)
 {
+    uint32_t z = x - y;
     if constexpr (DT == DT_F64) {
-        // one IEEE double multiply of an exactly converted integer (reading M3)
-        return (double)(z == 0 ? M1 : z) * 2.328306549295727688e-10;
+        if (x <= y) z += M1;
+        // one IEEE double multiply of an exactly converted integer
+        return (double)z * 2.328306549295727688e-10;
     } else {
+        if (x < y) z += M1;
         return convert<DT>(z);
     }
 }
@@ -116,39 +119,85 @@ mrg32k3a_jump_kernel(const uint32_t *__restrict__ base, const uint32_t *st_in,
     mrg_store(st_out, ns, s, r);
 }
 
-// One thread owns V adjacent streams and one row chunk (see k_lfsr113.cu for the mapping).
+__device__ __forceinline__ void mrg_apply_op(const MrgOp *__restrict__ op, Mrg &s)
+{
+    matvec3(op->a, s.x0, s.x1, s.x2, M1, C1);
+    matvec3(op->b, s.y0, s.y1, s.y2, M2, C2);
+}
+
+// One thread owns V adjacent streams and one row chunk: blockIdx.y = chunk c, so the row index is
+// uniform over the block.  Threads of a warp own adjacent stream groups: a warp writes 32*V
+// consecutive elements of a row per step (one 128-bit store per thread for V*sizeof(T) = 16).
+// The three-row body renames the state registers instead of moving them:
+//   (x_n, x_{n-1}, x_{n-2}) = (a,b,c) -> (c',a,b) -> (b',c',a) -> (a',b',c').
 template <int V, int DT>
 __global__ void __launch_bounds__(256)
 mrg32k3a_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
                     typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n,
-                    uint64_t chunk_len, uint64_t n_chunks, const MrgOp *__restrict__ chunk_ops)
+                    uint64_t chunk_len, const MrgOp *__restrict__ chunk_ops)
 {
     typedef typename OutElem<DT>::type T;
-    const uint64_t groups = ns / V;
-    const uint64_t vid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (vid >= groups * n_chunks) return;
-    const uint64_t c = vid / groups, sg = vid - c * groups;
+    const uint64_t sg = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint64_t s0 = sg * V;
+    if (s0 >= ns) return;
+    const uint32_t c = blockIdx.y;
 
     Mrg g[V];
 #pragma unroll
     for (int v = 0; v < V; v++) g[v] = mrg_load(st_in, ns, s0 + v);
     if (c != 0) {
 #pragma unroll
-        for (int v = 0; v < V; v++) mrg_apply_bits(chunk_ops, c, g[v]);
+        for (int v = 0; v < V; v++) mrg_apply_op(chunk_ops + (c - 1), g[v]);
     }
-    const uint64_t row0 = c * chunk_len;
-    const uint64_t row1 = (row0 + chunk_len < n) ? row0 + chunk_len : n;
+    const uint64_t row0 = (uint64_t)c * chunk_len;
+    const uint64_t rows = (row0 + chunk_len < n) ? chunk_len : n - row0;
     T *p = out + row0 * ns + s0;
-#pragma unroll 2
-    for (uint64_t i = row0; i < row1; i++) {
-        T r[V];
+    T r[V];
+    // the fold constants as opaque register values: as literals ptxas re-materialises them (one
+    // immediate per IMAD) inside the loop
+    uint32_t c1 = C1;
+    asm volatile("" : "+r"(c1));
+    uint64_t i = 0;
+#pragma unroll 1
+    for (; i + 3 <= rows; i += 3) {
 #pragma unroll
-        for (int v = 0; v < V; v++) r[v] = mrg_convert<DT>(mrg_step(g[v]));
+        for (int v = 0; v < V; v++) {
+            g[v].x2 = mrg_next_x(g[v].x1, g[v].x2, c1);
+            g[v].y2 = mrg_next_y(g[v].y0, g[v].y2);
+            r[v] = mrg_output<DT>(g[v].x2, g[v].y2);
+        }
+        store_vec<V>(p, r);
+        p += ns;
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            g[v].x1 = mrg_next_x(g[v].x0, g[v].x1, c1);
+            g[v].y1 = mrg_next_y(g[v].y2, g[v].y1);
+            r[v] = mrg_output<DT>(g[v].x1, g[v].y1);
+        }
+        store_vec<V>(p, r);
+        p += ns;
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            g[v].x0 = mrg_next_x(g[v].x2, g[v].x0, c1);
+            g[v].y0 = mrg_next_y(g[v].y1, g[v].y0);
+            r[v] = mrg_output<DT>(g[v].x0, g[v].y0);
+        }
         store_vec<V>(p, r);
         p += ns;
     }
-    if (c == n_chunks - 1) {
+#pragma unroll 1
+    for (; i < rows; i++) {                              // ragged tail: rotate by moving
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            uint32_t nx = mrg_next_x(g[v].x1, g[v].x2, c1), ny = mrg_next_y(g[v].y0, g[v].y2);
+            g[v].x2 = g[v].x1; g[v].x1 = g[v].x0; g[v].x0 = nx;
+            g[v].y2 = g[v].y1; g[v].y1 = g[v].y0; g[v].y0 = ny;
+            r[v] = mrg_output<DT>(nx, ny);
+        }
+        store_vec<V>(p, r);
+        p += ns;
+    }
+    if (c == gridDim.y - 1) {
 #pragma unroll
         for (int v = 0; v < V; v++) mrg_store(st_out, ns, s0 + v, g[v]);
     }
@@ -157,11 +206,11 @@ mrg32k3a_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
 template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
 {
     typedef typename OutElem<DT>::type T;
-    uint64_t threads = (a.n_streams / V) * a.n_chunks;
-    unsigned blocks = (unsigned)ceil_div_u64(threads, 256);
-    mrg32k3a_gen_kernel<V, DT><<<blocks, 256, 0, stream>>>(
+    const uint64_t groups = a.n_streams / V;
+    dim3 grid((unsigned)ceil_div_u64(groups, 256), (unsigned)a.n_chunks);
+    mrg32k3a_gen_kernel<V, DT><<<grid, 256, 0, stream>>>(
         (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
-        a.n_chunks, (const MrgOp *)a.chunk_ops);
+        (const MrgOp *)a.chunk_ops);
     return cudaGetLastError();
 }
 

@@ -103,6 +103,30 @@ int cuda_fail(cudaError_t e)
         if (e_ != cudaSuccess) return cuda_fail(e_);     \
     } while (0)
 
+// Device memory comes from the stream-ordered allocator (cudaMallocAsync on the default pool, kept
+// warm by a release threshold of "never"): init / free of a state cost microseconds and never
+// synchronise the device, so that prand_init + prand_generate + prand_free can be a hot loop.
+cudaError_t pool_setup()
+{
+    static cudaError_t status = [] {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        cudaMemPool_t pool;
+        e = cudaDeviceGetDefaultMemPool(&pool, dev);
+        if (e != cudaSuccess) return e;
+        uint64_t keep = UINT64_MAX;
+        return cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }();
+    return status;
+}
+cudaError_t dev_alloc(void **p, size_t bytes, cudaStream_t stream)
+{
+    cudaError_t e = pool_setup();
+    if (e != cudaSuccess) return e;
+    return cudaMallocAsync(p, bytes ? bytes : 1, stream);
+}
+
 }  // namespace
 
 struct prand_state {
@@ -117,13 +141,14 @@ struct prand_state {
     size_t ops_bytes;
     void *d_chunk_ops;      // cached operators for chunk_len * 2^j
     uint64_t chunk_len;
-    unsigned chunk_levels;
+    uint64_t chunk_count;   // operators cached for c = 1..chunk_count-1
     void *d_stage[2];       // device staging of the *_host calls
     size_t stage_bytes;
     cudaStream_t copy_stream;
     cudaEvent_t ev_gen[2], ev_copy[2];
     bool host_ready;
     const char *last_kernel;
+    cudaStream_t last_stream;   // stream of the most recent call: prand_free releases in its order
 };
 
 namespace {
@@ -131,8 +156,8 @@ namespace {
 int ensure_ops(prand_state *st, size_t bytes)
 {
     if (bytes <= st->ops_bytes) return PRAND_OK;
-    if (st->d_ops) { CU(cudaDeviceSynchronize()); CU(cudaFree(st->d_ops)); st->d_ops = nullptr; st->ops_bytes = 0; }
-    CU(cudaMalloc(&st->d_ops, bytes));
+    if (st->d_ops) { CU(cudaFreeAsync(st->d_ops, st->last_stream)); st->d_ops = nullptr; st->ops_bytes = 0; }
+    CU(dev_alloc(&st->d_ops, bytes, st->last_stream));
     st->ops_bytes = bytes;
     return PRAND_OK;
 }
@@ -140,7 +165,7 @@ int ensure_ops(prand_state *st, size_t bytes)
 int ensure_second_buffer(prand_state *st)
 {
     if (st->d_state[1 - st->cur]) return PRAND_OK;
-    CU(cudaMalloc(&st->d_state[1 - st->cur], st->bytes));
+    CU(dev_alloc(&st->d_state[1 - st->cur], st->bytes, st->last_stream));
     return PRAND_OK;
 }
 
@@ -295,15 +320,17 @@ int init_body(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
 void destroy(prand_state *st)
 {
     if (!st) return;
-    cudaDeviceSynchronize();
+    // stream-ordered release: everything this state launched was on last_stream (the *_host calls
+    // drain their copy stream before returning), so no device-wide synchronisation is needed
+    cudaStream_t s = st->last_stream;
     for (int i = 0; i < 2; i++) {
-        if (st->d_state[i]) cudaFree(st->d_state[i]);
-        if (st->d_stage[i]) cudaFree(st->d_stage[i]);
+        if (st->d_state[i]) cudaFreeAsync(st->d_state[i], s);
+        if (st->d_stage[i]) cudaFreeAsync(st->d_stage[i], s);
         if (st->host_ready) { cudaEventDestroy(st->ev_gen[i]); cudaEventDestroy(st->ev_copy[i]); }
     }
     if (st->host_ready) cudaStreamDestroy(st->copy_stream);
-    if (st->d_ops) cudaFree(st->d_ops);
-    if (st->d_chunk_ops) cudaFree(st->d_chunk_ops);
+    if (st->d_ops) cudaFreeAsync(st->d_ops, s);
+    if (st->d_chunk_ops) cudaFreeAsync(st->d_chunk_ops, s);
     delete st;
 }
 
@@ -337,8 +364,9 @@ extern "C" int prand_init_shard(prand_state **out, int gen, uint64_t seed, uint6
     st->first = first_stream;
     st->bytes = (size_t)n_streams * stream_bytes(gen);
     st->last_kernel = "";
+    st->last_stream = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaGetDevice(&st->device);
-    if (e == cudaSuccess) e = cudaMalloc(&st->d_state[0], st->bytes);
+    if (e == cudaSuccess) e = dev_alloc(&st->d_state[0], st->bytes, st->last_stream);
     if (e != cudaSuccess) {
         delete st;
         g_last_cuda_error = (int)e;
@@ -366,6 +394,7 @@ extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_l
     if (steps_log2 > 32768) return PRAND_ERR_ARG;
     if (steps_mant == 0) return PRAND_OK;
     cudaStream_t stream = (cudaStream_t)cuda_stream;
+    st->last_stream = stream;
     Dist n = {steps_mant, steps_log2};
     std::vector<unsigned char> ops;
     int rc = build_level_ops(st->gen, n, 1, ops);
@@ -422,31 +451,37 @@ void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t 
         }
         uint64_t threads = ns * lanes_per_stream / per_thread_streams;
         if (threads == 0) threads = 1;
-        const uint64_t target = (uint64_t)sms * 1024;
-        if (threads >= target) return;
-        uint64_t want = (target + threads - 1) / threads;
+        // one balanced wave: as many equal chunks as fit the threads resident at once, never more
+        // (a second, partial wave would cost a whole chunk time)
+        const uint64_t capacity = (uint64_t)sms * 1024;
+        if (2 * threads > capacity) return;
+        const uint64_t want = capacity / threads;
         len = (n + want - 1) / want;
         if (len < min_len) len = min_len;
     }
-    len = (len + 3) & ~3ull;                       // the 4-lane GM path stores rows in groups of four
+    len = (len + 11) / 12 * 12;                    // 4: row groups of the 4-lane GM path; 3: MRG32K3A's renamed rotation
     if (len >= n) return;
+    if ((n + len - 1) / len > 65535) len = ((n + 65534) / 65535 + 11) / 12 * 12;   // chunks ride on gridDim.y
     *chunk_len = len;
     *n_chunks = (n + len - 1) / len;
 }
 
 int ensure_chunk_ops(prand_state *st, uint64_t chunk_len, uint64_t n_chunks, cudaStream_t stream)
 {
-    const unsigned levels = bit_length(n_chunks - 1);
-    if (st->d_chunk_ops && st->chunk_len == chunk_len && st->chunk_levels >= levels) return PRAND_OK;
-    std::vector<unsigned char> ops;
-    Dist n = {chunk_len, 0};
-    int rc = build_level_ops(st->gen, n, levels, ops);
-    if (rc) return rc;
-    if (st->d_chunk_ops) { CU(cudaDeviceSynchronize()); CU(cudaFree(st->d_chunk_ops)); st->d_chunk_ops = nullptr; }
-    CU(cudaMalloc(&st->d_chunk_ops, ops.size()));
+    if (st->d_chunk_ops && st->chunk_len == chunk_len && st->chunk_count >= n_chunks) return PRAND_OK;
+    // operator of distance c * chunk_len for c = 1..n_chunks-1: one application per virtual stream
+    std::vector<unsigned char> ops, one;
+    for (uint64_t c = 1; c < n_chunks; c++) {
+        Dist d = {c * chunk_len, 0};
+        int rc = build_level_ops(st->gen, d, 1, one);
+        if (rc) return rc;
+        ops.insert(ops.end(), one.begin(), one.end());
+    }
+    if (st->d_chunk_ops) { CU(cudaFreeAsync(st->d_chunk_ops, stream)); st->d_chunk_ops = nullptr; }
+    CU(dev_alloc(&st->d_chunk_ops, ops.size(), stream));
     UPLOAD(st->d_chunk_ops, ops.data(), ops.size(), stream);
     st->chunk_len = chunk_len;
-    st->chunk_levels = levels;
+    st->chunk_count = n_chunks;
     return PRAND_OK;
 }
 
@@ -454,6 +489,7 @@ int generate(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t str
 {
     if (!st || (!out && n)) return PRAND_ERR_ARG;
     if (n == 0) return PRAND_OK;
+    st->last_stream = stream;
     const size_t esz = dtype == DT_F64 ? 8 : 4;
     if ((uintptr_t)out % esz) return PRAND_ERR_ARG;
     {
@@ -503,10 +539,9 @@ int ensure_host_path(prand_state *st, size_t want_bytes)
         st->host_ready = true;
     }
     if (st->stage_bytes < want_bytes) {
-        CU(cudaDeviceSynchronize());
-        for (int i = 0; i < 2; i++) {
-            if (st->d_stage[i]) { CU(cudaFree(st->d_stage[i])); st->d_stage[i] = nullptr; }
-            CU(cudaMalloc(&st->d_stage[i], want_bytes));
+        for (int i = 0; i < 2; i++) {      // earlier *_host calls drained both streams before returning
+            if (st->d_stage[i]) { CU(cudaFreeAsync(st->d_stage[i], st->last_stream)); st->d_stage[i] = nullptr; }
+            CU(dev_alloc(&st->d_stage[i], want_bytes, st->last_stream));
         }
         st->stage_bytes = want_bytes;
     }
@@ -517,6 +552,7 @@ int generate_host(prand_state *st, void *host_out, uint64_t n, int dtype, cudaSt
 {
     if (!st || (!host_out && n)) return PRAND_ERR_ARG;
     if (n == 0) return PRAND_OK;
+    st->last_stream = stream;
     const size_t esz = dtype == DT_F64 ? 8 : 4;
     const size_t row_bytes = (size_t)st->ns * esz;
     const size_t block_target = (size_t)256 << 20;
