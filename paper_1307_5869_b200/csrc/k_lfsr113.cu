@@ -57,21 +57,126 @@ lfsr113_jump_kernel(const uint32_t *__restrict__ base, const uint32_t *st_in,
     for (int c = 0; c < 4; c++) st_out[c * ns + s] = z[c];
 }
 
+// ---- bit-stream form of one component (hot path) -------------------------------------------------
+// Successive output words of a component overlap: word n is bits x_{ns}..x_{ns+31} of ONE bit
+// sequence, so an output consumes only s fresh bits (18 + 2 + 7 + 13 = 40 for the four components)
+// while the word form recomputes 4 x 5 shift/logic operations.  Here the sequence is kept as 32-bit
+// words W_j = x_{32j}..x_{32j+31} (MSB first) and extended a whole word at a time with eq. 9
+// (PAPER.md:363-368): x_n = x_{n-Kp} + x_{n-Kp+Kq} for K = 2^e.  A word needs K(p-q) >= 32 so that
+// every operand bit is already known: K = 2 for components 1, 2, 4 and K = 4 for component 3.
+// Each new word is two funnel shifts and one XOR; output n is one funnel shift at bit offset
+// n*s mod 32, a compile-time constant when 32 outputs are unrolled (after 32 outputs the offset is
+// back to 0 and the sequence has advanced exactly s words).  ~9.75 ALU operations per output
+// instead of 22.
+template <int R> __device__ __forceinline__ uint32_t funnel(uint32_t first, uint32_t second)
+{
+    // 32 bits starting R bits into the 64-bit string first:second (MSB first)
+    if constexpr (R == 0) return first;
+    else return __funnelshift_l(second, first, R);
+}
+
+template <int P, int Q, int S> struct TausBits {
+    static constexpr int K = (2 * (P - Q) >= 32) ? 2 : 4;
+    static constexpr int H = K;                                     // ring of history words
+    static constexpr int R1 = 32 * K - K * P, R2 = R1 + K * Q;      // bit offsets of the two taps from word j-K
+    static_assert(K * (P - Q) >= 32 && R1 >= 0 && R2 + 32 <= 32 * K, "eq. 9 taps must lie in known words");
+    uint32_t w[H];                                                  // word j lives in w[j % H]
+
+    __host__ __device__ static constexpr int need(int n) { return (n * S + 31) / 32; }  // last word output n touches
+    __host__ __device__ static constexpr int upto(int n) { return need(n) > H - 1 ? need(n) : H - 1; }
+
+    // (v, valid): the top `valid` bits of v are sequence bits; extend to `target` bits with eq. 7
+    __device__ static __forceinline__ uint64_t extend(uint64_t v, int valid, int target)
+    {
+        while (valid < target) {
+            int g = (P - Q < target - valid) ? P - Q : target - valid;
+            uint64_t t = (v >> P) ^ (v >> (P - Q));                 // bit index i holds x_{i-P} ^ x_{i-P+Q}
+            uint64_t m = (~0ull >> valid) & ~((valid + g >= 64) ? 0ull : (~0ull >> (valid + g)));
+            v |= t & m;
+            valid += g;
+        }
+        return v;
+    }
+    // from the state word z (top P bits significant): words 0..H-1 of the sequence starting at z
+    __device__ __forceinline__ void load(uint32_t z)
+    {
+        constexpr uint32_t top_p = 0xFFFFFFFFu << (32 - P);
+        uint64_t v = extend((uint64_t)(z & top_p) << 32, P, 64);
+        w[0] = (uint32_t)(v >> 32);
+        w[1] = (uint32_t)v;
+#pragma unroll
+        for (int j = 2; j < H; j++) w[j] = (uint32_t)extend((uint64_t)w[j - 1] << 32, 32, 64);
+    }
+    template <int J> __device__ __forceinline__ void gen()          // word J from words J-K..J-1
+    {
+        constexpr int A1 = J - K + (R1 >> 5), A2 = J - K + (R2 >> 5);
+        uint32_t t1 = funnel<(R1 & 31)>(w[A1 % H], w[(A1 + 1) % H]);
+        uint32_t t2 = funnel<(R2 & 31)>(w[A2 % H], w[(A2 + 1) % H]);
+        w[J % H] = t1 ^ t2;
+    }
+    template <int J0, int J1> __device__ __forceinline__ void gen_range()
+    {
+        if constexpr (J0 <= J1) { gen<J0>(); gen_range<J0 + 1, J1>(); }
+    }
+    // output N = 1..32 of the current block (step-then-output: output N is the word at bit N*S)
+    template <int N> __device__ __forceinline__ uint32_t output()
+    {
+        gen_range<upto(N - 1) + 1, upto(N)>();
+        constexpr int a = (N * S) / 32, r = (N * S) % 32;
+        return funnel<r>(w[a % H], w[(a + 1) % H]);
+    }
+    // after output 32 the sequence has advanced S words: make word S the new word 0
+    __device__ __forceinline__ void next_block()
+    {
+        gen_range<upto(32) + 1, S + H - 1>();
+        uint32_t t[H];
+#pragma unroll
+        for (int i = 0; i < H; i++) t[i] = w[(S + i) % H];
+#pragma unroll
+        for (int i = 0; i < H; i++) w[i] = t[i];
+    }
+    __device__ __forceinline__ uint32_t state() const { return w[0]; }   // all 32 bits are sequence bits
+};
+
+template <int V> struct LfsrBits {
+    TausBits<31, 6, 18> c1[V];
+    TausBits<29, 2, 2> c2[V];
+    TausBits<28, 13, 7> c3[V];
+    TausBits<25, 3, 13> c4[V];
+};
+
+template <int V, int DT, int N>
+__device__ __forceinline__ void lfsr113_emit_rows(LfsrBits<V> &b, typename OutElem<DT>::type *&p, uint64_t ns)
+{
+    if constexpr (N <= 32) {
+        typename OutElem<DT>::type r[V];
+#pragma unroll
+        for (int v = 0; v < V; v++)
+            r[v] = convert<DT>(b.c1[v].template output<N>() ^ b.c2[v].template output<N>() ^
+                               b.c3[v].template output<N>() ^ b.c4[v].template output<N>());
+        store_vec<V>(p, r);
+        p += ns;
+        lfsr113_emit_rows<V, DT, N + 1>(b, p, ns);
+    }
+}
+
 // One thread owns V adjacent streams (V = 4: one 128-bit store per row for u32/f32, two for f64)
-// and one row chunk.  Threads of a warp own adjacent stream groups, so a warp writes 32*V
-// consecutive elements of a row per step.
+// and one row chunk (blockIdx.y).  Threads of a warp own adjacent stream groups, so a warp writes
+// 32*V consecutive elements of a row per step.  Rows go out in blocks of 32 in the bit-stream form;
+// a ragged tail (< 32 rows) uses the word form.
+constexpr int GEN_THREADS = 128;
+
 template <int V, int DT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(GEN_THREADS)
 lfsr113_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
                    typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n,
-                   uint64_t chunk_len, uint64_t n_chunks, const LfsrOp *__restrict__ chunk_ops)
+                   uint64_t chunk_len, const LfsrOp *__restrict__ chunk_ops)
 {
     typedef typename OutElem<DT>::type T;
-    const uint64_t groups = ns / V;
-    const uint64_t vid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (vid >= groups * n_chunks) return;
-    const uint64_t c = vid / groups, sg = vid - c * groups;
+    const uint64_t sg = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint64_t s0 = sg * V;
+    if (s0 >= ns) return;
+    const uint32_t c = blockIdx.y;
 
     uint32_t z[V][4];
 #pragma unroll
@@ -88,18 +193,34 @@ lfsr113_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
 #pragma unroll
         for (int v = 0; v < V; v++) lfsr113_apply_bits(chunk_ops + (c - 1), 1, z[v]);   // operator of c * chunk_len
     }
-    const uint64_t row0 = c * chunk_len;
-    const uint64_t row1 = (row0 + chunk_len < n) ? row0 + chunk_len : n;
+    const uint64_t row0 = (uint64_t)c * chunk_len;
+    const uint64_t rows = (row0 + chunk_len < n) ? chunk_len : n - row0;
     T *p = out + row0 * ns + s0;
-#pragma unroll 4
-    for (uint64_t i = row0; i < row1; i++) {
+    const uint64_t blocks32 = rows / 32;
+    if (blocks32) {
+        LfsrBits<V> b;
+#pragma unroll
+        for (int v = 0; v < V; v++) { b.c1[v].load(z[v][0]); b.c2[v].load(z[v][1]); b.c3[v].load(z[v][2]); b.c4[v].load(z[v][3]); }
+#pragma unroll 1
+        for (uint64_t blk = 0; blk < blocks32; blk++) {
+            lfsr113_emit_rows<V, DT, 1>(b, p, ns);
+#pragma unroll
+            for (int v = 0; v < V; v++) { b.c1[v].next_block(); b.c2[v].next_block(); b.c3[v].next_block(); b.c4[v].next_block(); }
+        }
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            z[v][0] = b.c1[v].state(); z[v][1] = b.c2[v].state(); z[v][2] = b.c3[v].state(); z[v][3] = b.c4[v].state();
+        }
+    }
+#pragma unroll 1
+    for (uint64_t i = blocks32 * 32; i < rows; i++) {
         T r[V];
 #pragma unroll
         for (int v = 0; v < V; v++) r[v] = convert<DT>(lfsr113_step(z[v]));
         store_vec<V>(p, r);
         p += ns;
     }
-    if (c == n_chunks - 1) {
+    if (c == gridDim.y - 1) {
 #pragma unroll
         for (int k = 0; k < 4; k++)
 #pragma unroll
@@ -111,11 +232,10 @@ template <int V, int DT>
 cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
 {
     typedef typename OutElem<DT>::type T;
-    uint64_t threads = (a.n_streams / V) * a.n_chunks;
-    unsigned blocks = (unsigned)ceil_div_u64(threads, 256);
-    lfsr113_gen_kernel<V, DT><<<blocks, 256, 0, stream>>>(
+    dim3 grid((unsigned)ceil_div_u64(a.n_streams / V, GEN_THREADS), (unsigned)a.n_chunks);
+    lfsr113_gen_kernel<V, DT><<<grid, GEN_THREADS, 0, stream>>>(
         (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
-        a.n_chunks, (const LfsrOp *)a.chunk_ops);
+        (const LfsrOp *)a.chunk_ops);
     return cudaGetLastError();
 }
 

@@ -14,6 +14,8 @@ namespace {
 
 constexpr uint32_t M1 = 4294967087u, M2 = 4294944443u;
 constexpr uint32_t C1 = 209u, C2 = 22853u;
+// small CTAs: with ~1000 CTAs on 148 SMs the most loaded SM is within 2% of the average
+constexpr int GEN_THREADS = 128;
 
 struct Mrg { uint32_t x0, x1, x2, y0, y1, y2; };   // x0 = x_n, x1 = x_{n-1}, x2 = x_{n-2}
 
@@ -131,7 +133,7 @@ __device__ __forceinline__ void mrg_apply_op(const MrgOp *__restrict__ op, Mrg &
 // The three-row body renames the state registers instead of moving them:
 //   (x_n, x_{n-1}, x_{n-2}) = (a,b,c) -> (c',a,b) -> (b',c',a) -> (a',b',c').
 template <int V, int DT>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(GEN_THREADS)
 mrg32k3a_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
                     typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n,
                     uint64_t chunk_len, const MrgOp *__restrict__ chunk_ops)
@@ -207,8 +209,8 @@ template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenAr
 {
     typedef typename OutElem<DT>::type T;
     const uint64_t groups = a.n_streams / V;
-    dim3 grid((unsigned)ceil_div_u64(groups, 256), (unsigned)a.n_chunks);
-    mrg32k3a_gen_kernel<V, DT><<<grid, 256, 0, stream>>>(
+    dim3 grid((unsigned)ceil_div_u64(groups, GEN_THREADS), (unsigned)a.n_chunks);
+    mrg32k3a_gen_kernel<V, DT><<<grid, GEN_THREADS, 0, stream>>>(
         (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
         (const MrgOp *)a.chunk_ops);
     return cudaGetLastError();

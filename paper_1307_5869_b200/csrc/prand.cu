@@ -459,9 +459,12 @@ void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t 
         len = (n + want - 1) / want;
         if (len < min_len) len = min_len;
     }
-    len = (len + 11) / 12 * 12;                    // 4: row groups of the 4-lane GM path; 3: MRG32K3A's renamed rotation
+    // whole row blocks per chunk: 32 for LFSR113's bit-stream form, else 12 (4: row groups of the
+    // 4-lane GM path; 3: MRG32K3A's renamed rotation)
+    const uint64_t gran = gen == PRAND_LFSR113 ? 32 : 12;
+    len = (len + gran - 1) / gran * gran;
     if (len >= n) return;
-    if ((n + len - 1) / len > 65535) len = ((n + 65534) / 65535 + 11) / 12 * 12;   // chunks ride on gridDim.y
+    if ((n + len - 1) / len > 65535) len = ((n + 65534) / 65535 + gran - 1) / gran * gran;   // chunks ride on gridDim.y
     *chunk_len = len;
     *n_chunks = (n + len - 1) / len;
 }
