@@ -197,7 +197,8 @@ def run_ours(args, w):
     gen_fn = {"u32": P.prand_generate_u32, "f32": P.prand_generate_f32, "f64": P.prand_generate_f64}[w.dtype]
     host_fn = {"u32": P.prand_generate_u32_host, "f32": P.prand_generate_f32_host,
                "f64": P.prand_generate_f64_host}[w.dtype]
-    first = rank * w.n_streams                     # weak scaling: rank r holds streams [r ns, (r+1) ns)
+    from paper_1307_5869_b200 import sharding
+    first, _ = sharding.weak_shard(w.n_streams, rank)   # weak scaling: rank r holds streams [r ns, (r+1) ns)
     out = torch.empty((w.n_per_stream, w.n_streams), dtype=tdt, device="cuda")
     need_flush = w.out_bytes <= (1 << 30)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if need_flush else None
@@ -237,10 +238,7 @@ def run_ours(args, w):
     else:
         elapsed_ms = t_all0.elapsed_time(t_all1)
     kernel_ms = [a.elapsed_time(b) for a, b in kev]
-    if dist is not None:
-        t = torch.tensor([elapsed_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        elapsed_ms = float(t.item())
+    elapsed_ms = sharding.max_over_ranks(elapsed_ms, device="cuda")
     ms_per_step = elapsed_ms / args.steps
     value = world * w.numbers / (ms_per_step * 1e-3) / 1e9
 
@@ -280,10 +278,7 @@ def run_ours(args, w):
         barrier()
         wall_ms = (time.perf_counter() - t0) * 1e3
         ev_ms = max(a.elapsed_time(b), wall_ms)      # the call returns after the data arrived: both agree
-        if dist is not None:
-            t = torch.tensor([ev_ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ev_ms = float(t.item())
+        ev_ms = sharding.max_over_ranks(ev_ms, device="cuda")
         e2e = {"value": world * w.numbers * ke / (ev_ms * 1e-3) / 1e9, "unit": UNIT,
                "h2d_bytes_per_step": (P.prand_uploaded_bytes() - up0) // ke,
                "d2h_bytes_per_step": w.out_bytes, "steps": ke, "warmup": 1, "ms_per_step": ev_ms / ke,
