@@ -7,6 +7,7 @@
 //   x_{i+624} = x_{i+397} ^ (y >> 1) ^ (y odd ? 0x9908B0DF : 0),  y = (x_i & 0x80000000) | (x_{i+1} & 0x7FFFFFFF),
 // output number P = temper(x_{P+624}); the state at position P is the window x_P..x_{P+623}.
 // State layout: [stream][624] u32 (one stream's window is contiguous: a warp loads it coalesced).
+#include <cstdlib>
 #include "k_common.cuh"
 
 namespace prand {
@@ -18,14 +19,6 @@ __device__ __forceinline__ uint32_t mt_recur(uint32_t xi, uint32_t xi1, uint32_t
 {
     uint32_t y = (xi & 0x80000000u) | (xi1 & 0x7FFFFFFFu);
     return xim ^ (y >> 1) ^ ((0u - (y & 1u)) & 0x9908B0DFu);
-}
-__device__ __forceinline__ uint32_t mt_temper(uint32_t y)
-{
-    y ^= y >> 11;
-    y ^= (y << 7) & 0x9D2C5680u;
-    y ^= (y << 15) & 0xEFC60000u;
-    y ^= y >> 18;
-    return y;
 }
 
 // ---- eq. 10 in correlation form -----------------------------------------------------------------
@@ -77,84 +70,403 @@ mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
 }
 
 // ---- generation ----------------------------------------------------------------------------------
-// CTA = G warps; warp w owns stream s0 + w with its 624-word window as a circular buffer in shared
-// memory; lane l produces x_{P+624+l}, 32 new words per round (the recurrence reaches back 227 >= 32
-// words, so a round's 32 words are independent).  Rounds of all G warps are transposed through a
-// [32][G] tile so that each output row segment out[i*ns + s0 .. s0+G) is written contiguously.
-template <int G, int DT>
-__global__ void __launch_bounds__(G * 32)
-mt19937_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
-                   typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n)
+// CTA = S adjacent streams x T word slices (thread = (slice t, stream ls), ls fastest).  Thread
+// (t, ls) owns the K = 624/T words w = T j + t, j = 0..K-1, of stream ls and keeps them in registers.
+// One *round* regenerates the whole window (624 new numbers per stream): word w of the new window is
+//     x'_w = x_{w+397} ^ twist(x_w, x_{w+1})            for w < 227  (all inputs from the old window)
+//     x'_w = x'_{w-227} ^ twist(x_w, x_{w+1})           for w >= 227 (x_{w+1} = x'_0 for w = 623)
+// so any 227 consecutive words are independent of each other (the 227 of PAPER.md:400, Table 5):
+// M waves of T words (T M <= 227) run between two CTA barriers, every thread is busy in every wave.
+// The neighbour words come from shared memory, which holds the old and the new window
+// ([2][S][P] words, P = 624 + pad chosen so that both the generation pattern -- a warp reads 32/S
+// consecutive words of S streams -- and the coalesced state load/store pattern are bank-conflict
+// free).  A warp's store covers 32/S rows x S adjacent streams: full 32-byte sectors for S = 8.
+// With few streams (C3: 512) S = 4 keeps 128 CTAs busy; the two CTAs that share a 32-byte sector form
+// a cluster and meet at a cluster barrier once per round so that L2 merges their half-sector writes.
+template <int S> struct MtPitch { static constexpr int value = 624 + 16 + (32 / S) % 32; };   // = 32/S mod 32, multiple of 4
+template <> struct MtPitch<1> { static constexpr int value = 640; };
+
+// Arithmetic of one number, arranged for the B200 pipes.  The ALU pipe (LOP3, SHF:
+// 64 lanes/clk/SM) is the binding one, so everything that is not a logic operation runs on the
+// FMA-heavy pipe: with rot = rotr(y, 1) the twist is
+//     (y >> 1) ^ (y odd ? 0x9908B0DF : 0) = rot ^ (y odd ? 0x1908B0DF : 0)
+// (the rotation already puts y's low bit into bit 31), and the second term is
+// mul.hi(x1 << 31, 2 * 0x1908B0DF): IMAD.SHL + IMAD.HI.  Right shifts of the tempering can run as
+// mul.hi by 2^(32-r) (HI bit 1: >> 11, bit 2: >> 18).  The multipliers are kernel arguments so that
+// ptxas cannot turn them back into shifts or selects.  Per number: 3 + 4 LOP3/SHF, 1 address add.
+struct MtMul { uint32_t a2, m31, m21, m14; };
+
+__device__ __forceinline__ uint32_t lop3_e4(uint32_t a, uint32_t b, uint32_t c)   // (a & c) | (b & ~c)
 {
-    typedef typename OutElem<DT>::type T;
-    constexpr int PITCH = G + 1;
-    extern __shared__ uint32_t smem[];
-    uint32_t *xs = smem;                       // [G][NW]
-    uint32_t *tile = smem + G * NW;            // [2][32][PITCH]
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint64_t s0 = (uint64_t)blockIdx.x * G;
-    const uint64_t s = s0 + warp;
-    const bool live = s < ns;
-    uint32_t *x = xs + warp * NW;
-    if (live)
-        for (int j = lane; j < NW; j += 32) x[j] = st_in[s * NW + j];
-    __syncwarp();
-    int h = 0;                                 // slot of x_P
-    int buf = 0;
-    for (uint64_t t0 = 0; t0 < n; t0 += 32, buf ^= 1) {
-        const int rem = (n - t0 < 32) ? (int)(n - t0) : 32;
-        uint32_t *tl = tile + buf * 32 * PITCH;
-        if (live) {
-            int a = h + lane;      if (a >= NW) a -= NW;
-            int b = a + 1;         if (b >= NW) b -= NW;
-            int m = a + MW;        if (m >= NW) m -= NW;
-            uint32_t nw = mt_recur(x[a], x[b], x[m]);
-            __syncwarp();
-            if (lane < rem) x[a] = nw;
-            __syncwarp();
-            tl[lane * PITCH + warp] = mt_temper(nw);
-            h += rem; if (h >= NW) h -= NW;
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+
+template <int HI, int BIT> __device__ __forceinline__ uint32_t mt_shr(uint32_t x, int r, uint32_t mul)
+{
+    return ((HI >> BIT) & 1) ? __umulhi(x, mul) : (x >> r);
+}
+
+template <int HI> __device__ __forceinline__ uint32_t mt_recur2(uint32_t x0, uint32_t x1, uint32_t xm, const MtMul &c)
+{
+    const uint32_t y = lop3_e4(x0, x1, 0x80000000u);
+    const uint32_t rot = __funnelshift_r(y, y, 1);
+    const uint32_t h = __umulhi(x1 * c.m31, c.a2);
+    return xor3(xm, rot, h);
+}
+template <int HI> __device__ __forceinline__ uint32_t mt_temper2(uint32_t y, const MtMul &c)
+{
+    y ^= mt_shr<HI, 1>(y, 11, c.m21);
+    y ^= (y << 7) & 0x9D2C5680u;
+    y ^= (y << 15) & 0xEFC60000u;
+    y ^= mt_shr<HI, 2>(y, 18, c.m14);
+    return y;
+}
+
+__device__ __forceinline__ void cluster_arrive()
+{
+    asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_wait()
+{
+    asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
+}
+
+// One round (FULL) or the first `rem` words of one (the tail of a call).  ob = this thread's byte
+// offset (row t, stream s) from the uniform row-block pointer `rows`.
+template <int S, int T, int M, int DT, int HI, bool FULL, bool ALL>
+__device__ __forceinline__ void mt_round(uint32_t *smem, const uint32_t ia, const uint32_t ib, const int t,
+                                         uint32_t (&r)[NW / T], char *rows, const uint32_t ob,
+                                         const uint64_t wave_bytes, const bool live, const int rem,
+                                         const MtMul &c)
+{
+    typedef typename OutElem<DT>::type E;
+    constexpr int K = NW / T;
+#pragma unroll
+    for (int j = 0; j < K; j++) {
+        const int w = T * j + t;
+        if (FULL || w < rem) {
+            const uint32_t x1 = smem[ia + T * j + 1];
+            uint32_t xm;
+            if (T * (j + 1) <= NW - MW) xm = smem[ia + T * j + MW];
+            else if (T * j >= NW - MW) xm = smem[ib + T * j - (NW - MW)];
+            else xm = smem[(w < NW - MW ? ia + MW : ib - (NW - MW)) + T * j];
+            const uint32_t nw = mt_recur2<HI>(r[j], x1, xm, c);
+            r[j] = nw;
+            smem[ib + T * j] = nw;
+            if (j == 0 && t == 0) smem[ia + NW] = nw;       // x_{w+1} of word 623 is the new word 0
+            const E v = convert<DT>(mt_temper2<HI>(nw, c));
+            if (ALL || live) store1(reinterpret_cast<E *>(rows + j * wave_bytes + ob), v);
         }
-        __syncthreads();
-        {
-            const int row = threadIdx.x / G, col = threadIdx.x % G;
-            if (row < rem && s0 + col < ns)
-                store1(out + (t0 + row) * ns + s0 + col, convert<DT>(tl[row * PITCH + col]));
+        if ((j + 1) % M == 0) __syncthreads();
+    }
+}
+
+template <int S, int T, int M, int DT, int HI, bool PAIR>
+__global__ void __launch_bounds__(S * T)
+mt19937_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
+                   typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n, const MtMul c)
+{
+    typedef typename OutElem<DT>::type E;
+    constexpr int K = NW / T, P = MtPitch<S>::value, NT = S * T;
+    static_assert(NW % T == 0 && K % M == 0 && T * M <= NW - MW, "bad MT19937 tiling");
+    static_assert(P % 4 == 0 && P > NW, "bad pitch");
+    extern __shared__ __align__(16) uint32_t smem[];     // [2][S][P]
+    const int tid = threadIdx.x, ls = tid % S, t = tid / S;
+    const uint64_t s0 = (uint64_t)blockIdx.x * S;
+    const uint64_t s = s0 + ls;
+    const bool live = s < ns;
+    const int n_live = s0 >= ns ? 0 : (ns - s0 < (uint64_t)S ? (int)(ns - s0) : S);
+
+    // state load: the CTA's S windows are one contiguous piece of st_in
+    for (int i = tid; i < S * (NW / 4); i += NT) {
+        const int q = i / (NW / 4), w4 = i % (NW / 4);
+        if (q < n_live) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4 *>(st_in + (s0 + q) * NW) + w4);
+            *reinterpret_cast<uint4 *>(smem + q * P + 4 * w4) = v;
         }
     }
-    if (live) {
-        __syncwarp();
-        for (int j = lane; j < NW; j += 32) {
-            int a = h + j; if (a >= NW) a -= NW;
-            uint32_t v = x[a];
-            st_out[s * NW + j] = v;
+    __syncthreads();
+    uint32_t ia = ls * P + t, ib = ia + S * P;
+    uint32_t r[K];
+#pragma unroll
+    for (int j = 0; j < K; j++) r[j] = smem[ia + T * j];
+    // the launcher guarantees (T * ns + S) * sizeof(E) < 2^32
+    const uint32_t ob = (uint32_t)(((uint64_t)t * ns + ls) * sizeof(E));
+    char *rows = reinterpret_cast<char *>(out + s0);
+    const uint64_t wave_bytes = (uint64_t)T * ns * sizeof(E);
+    const uint64_t round_bytes = (uint64_t)NW * ns * sizeof(E);
+    uint64_t left = n;
+    uint32_t cur = 0;                                     // buffer that holds the old window
+    bool pending = false;
+    if (n_live == S) {
+        while (left >= NW) {
+            mt_round<S, T, M, DT, HI, true, true>(smem, ia, ib, t, r, rows, ob, wave_bytes, true, NW, c);
+            if (PAIR) {                                   // stay within one round of the sector partner
+                if (pending) cluster_wait();
+                cluster_arrive();
+                pending = true;
+            }
+            const uint32_t tmp = ia; ia = ib; ib = tmp;
+            cur ^= 1;
+            rows += round_bytes;
+            left -= NW;
+        }
+    } else {
+        while (left >= NW) {
+            mt_round<S, T, M, DT, HI, true, false>(smem, ia, ib, t, r, rows, ob, wave_bytes, live, NW, c);
+            if (PAIR) {
+                if (pending) cluster_wait();
+                cluster_arrive();
+                pending = true;
+            }
+            const uint32_t tmp = ia; ia = ib; ib = tmp;
+            cur ^= 1;
+            rows += round_bytes;
+            left -= NW;
+        }
+    }
+    if (PAIR && pending) cluster_wait();
+    const int rem = (int)left;
+    if (rem) mt_round<S, T, M, DT, HI, false, false>(smem, ia, ib, t, r, rows, ob, wave_bytes, live, rem, c);
+    // final window x_{P+n}..x_{P+n+623}: words [rem, 624) of the old buffer, then [0, rem) of the new
+    const uint32_t *a0 = smem + cur * (S * P), *b0 = smem + (cur ^ 1) * (S * P);
+    for (int i = tid; i < S * NW; i += NT) {
+        const int q = i / NW, j = i % NW;
+        if (q < n_live) {
+            const int p = j + rem;
+            st_out[(s0 + q) * NW + j] = p < NW ? a0[q * P + p] : b0[q * P + p - NW];
         }
     }
 }
 
-template <int G, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
+template <int S, int T, int M, int DT, int HI, bool PAIR> cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
 {
-    typedef typename OutElem<DT>::type T;
-    size_t smem = (size_t)(G * NW + 2 * 32 * (G + 1)) * sizeof(uint32_t);
+    typedef typename OutElem<DT>::type E;
+    auto kern = mt19937_gen_kernel<S, T, M, DT, HI, PAIR>;
+    const size_t smem = (size_t)2 * S * MtPitch<S>::value * sizeof(uint32_t);
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(mt19937_gen_kernel<G, DT>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
-    unsigned blocks = (unsigned)ceil_div_u64(a.n_streams, G);
-    mt19937_gen_kernel<G, DT><<<blocks, G * 32, smem, stream>>>((const uint32_t *)a.st_in, (uint32_t *)a.st_out,
-                                                              (T *)a.out, a.n_streams, a.n);
+    uint64_t blocks = ceil_div_u64(a.n_streams, S);
+    if (PAIR) blocks += blocks & 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks);
+    cfg.blockDim = dim3(S * T);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = PAIR ? 2 : 1;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const MtMul c = {2u * 0x1908B0DFu, 1u << 31, 1u << 21, 1u << 14};
+    return cudaLaunchKernelEx(&cfg, kern, (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (E *)a.out,
+                              a.n_streams, a.n, c);
+}
+
+template <int S, int T, int M, int HI, bool PAIR> cudaError_t dispatch_dt(cudaStream_t stream, const GenArgs &a)
+{
+    switch (a.dtype) {
+    case DT_U32: return launch_gen<S, T, M, DT_U32, HI, PAIR>(stream, a);
+    case DT_F32: return launch_gen<S, T, M, DT_F32, HI, PAIR>(stream, a);
+    default: return launch_gen<S, T, M, DT_F64, HI, PAIR>(stream, a);
+    }
+}
+
+// ---- generation, many streams: lane = stream, one CTA per 32 streams --------------------------------
+// With thousands of streams a CTA can own 32 whole streams.  A window is a circular buffer in shared
+// memory regenerated *in place*: cell c always holds the latest x_n with n = c (mod 624), so x_{n+397}
+// is cell (c + 397) mod 624 whether it belongs to the old or the new window.  One round = three
+// intervals of 208 consecutive words (at most 227, see above); the CTA's 8 warps take the 8 slices of
+// an interval, warp u the 26 consecutive words base + 26 u ... of its 32 streams (lane = stream): x_w
+// of step i+1 is x_{w+1} of step i (a register), so a number costs two shared loads and one shared
+// store at compile-time offsets, each one conflict-free wavefront (pitch 625 is odd), and a warp
+// store is one full 128-byte line of a row: 4 L1 wavefronts per 32 numbers (the S = 8 kernels above
+// need 7, which is what bounds them).  Warps meet at a CTA barrier between intervals; inside one a
+// thread runs 2 x 13 independent recurrences.  80 KB of shared memory per CTA, two CTAs per SM.
+constexpr int WCH = 13;                                   // steps per chunk (operands staged in registers)
+
+// 13 consecutive steps of one slice.  a = cell of the first word, am = a + (397 or -227) for the
+// lanes' x_{w+397} cell; LAST: the chunk ends the slice, whose last x_{w+1} is the saved xb.
+template <int DT, int HI, bool GUARD, bool ALL, bool LAST>
+__device__ __forceinline__ void mt_chunk(uint32_t *a, const uint32_t *am, const uint32_t *am2, const int k2,
+                                         uint32_t &x0, const uint32_t xb, typename OutElem<DT>::type *&p,
+                                         const uint64_t ns, const bool live, const int left, const MtMul &c)
+{
+    typedef typename OutElem<DT>::type E;
+    // all operands first (none of these cells is written during the chunk before it is read), so that
+    // the 26 shared loads overlap and the 13 recurrences are independent instruction streams
+    uint32_t x[WCH + 1], xm[WCH];
+    x[0] = x0;
+#pragma unroll
+    for (int k = 0; k < WCH; k++) {
+        x[k + 1] = (LAST && k == WCH - 1) ? xb : a[k + 1];
+        xm[k] = (k >= k2 ? am2 : am)[k];
+    }
+#pragma unroll
+    for (int k = 0; k < WCH; k++) xm[k] = mt_recur2<HI>(x[k], x[k + 1], xm[k], c);
+#pragma unroll
+    for (int k = 0; k < WCH; k++)
+        if (!GUARD || k < left) a[k] = xm[k];
+#pragma unroll
+    for (int k = 0; k < WCH; k++) {
+        const E v = convert<DT>(mt_temper2<HI>(xm[k], c));
+        if ((!GUARD || k < left) && (ALL || live)) store1(p, v);
+        p += ns;
+    }
+    x0 = x[WCH];
+}
+
+// One interval: words [BASE + 39 u, BASE + 39 u + 39) for slice u.  GUARD: only words < rem are real (tail).
+template <bool CTA> __device__ __forceinline__ void mt_sync()
+{
+    if (CTA) __syncthreads(); else __syncwarp();
+}
+
+template <int BASE, int WB, int NSL, bool CTA, int DT, int HI, bool GUARD, bool ALL>
+__device__ __forceinline__ void mt_interval(uint32_t *A, const int u, typename OutElem<DT>::type *rowp,
+                                            const uint64_t ns, const bool live, const int rem, const MtMul &c)
+{
+    typedef typename OutElem<DT>::type E;
+    static_assert(WB % WCH == 0 && NSL * WB <= NW - MW && BASE + NSL * WB <= NW, "bad interval");
+    constexpr int NCH = WB / WCH, SW = NW - MW;           // x_{w+397} wraps to cell w - 227 from w = 227 on
+    const int w0 = BASE + WB * u;
+    // x_{w+1} of the slice's last word belongs to the next slice: read it before that slice overwrites it
+    const int wb = w0 + WB;
+    const uint32_t xb = A[wb == NW ? 0 : wb];
+    mt_sync<CTA>();
+    E *p = rowp + (uint64_t)w0 * ns;
+    asm("" : "+l"(p));                                    // one running pointer, not rowp + two offsets
+    uint32_t *a = A + w0;
+    uint32_t x0 = a[0];
+    // Only the interval that contains word 227 needs per-lane offsets, and only one slice of it switches
+    // inside its words: offsets are per-lane registers, the switch position is a compile-time step of
+    // the last chunk (u1 = the slice that contains word 227, k1 = its step within the last chunk).
+    constexpr bool STRADDLE = BASE < SW && BASE + NSL * WB > SW;
+    constexpr int u1 = STRADDLE ? (SW - BASE) / WB : 0, i1 = STRADDLE ? (SW - BASE) % WB : 0;
+    static_assert(!STRADDLE || i1 >= (NCH - 1) * WCH, "the switch must fall into the slice's last chunk");
+    const uint32_t *am, *am2;
+    int k2 = WCH;
+    if (!STRADDLE) {
+        am = am2 = a + (BASE < SW ? MW : -SW);
+    } else {
+        am = a + (u <= u1 ? MW : -SW);
+        am2 = a + (u < u1 ? MW : -SW);
+        k2 = i1 - (NCH - 1) * WCH;
+    }
+    int left = rem - w0;
+#pragma unroll 1
+    for (int ch = 0; ch < NCH - 1; ch++) {
+        mt_chunk<DT, HI, GUARD, ALL, false>(a, am, am, WCH, x0, xb, p, ns, live, left, c);
+        a += WCH; am += WCH; am2 += WCH; left -= WCH;
+    }
+    mt_chunk<DT, HI, GUARD, ALL, true>(a, am, am2, k2, x0, xb, p, ns, live, left, c);
+    mt_sync<CTA>();
+}
+
+constexpr int BP = 625;                                   // window pitch (odd: lane = stream is conflict-free)
+constexpr int BW = 8;                                     // warps per CTA = slices per interval
+constexpr int BSL = 26;                                   // words per slice per interval
+
+template <int DT, int HI, bool GUARD, bool ALL>
+__device__ __forceinline__ void mt_bround(uint32_t *A, const int u, typename OutElem<DT>::type *rowp,
+                                          const uint64_t ns, const bool live, const int rem, const MtMul &c)
+{
+    mt_interval<0, BSL, BW, true, DT, HI, GUARD, ALL>(A, u, rowp, ns, live, rem, c);
+    mt_interval<208, BSL, BW, true, DT, HI, GUARD, ALL>(A, u, rowp, ns, live, rem, c);
+    mt_interval<416, BSL, BW, true, DT, HI, GUARD, ALL>(A, u, rowp, ns, live, rem, c);
+}
+
+template <int DT, int HI>
+__global__ void __launch_bounds__(BW * 32, 2)
+mt19937_bgen_kernel(const uint32_t *st_in, uint32_t *st_out,
+                    typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n, const MtMul c)
+{
+    typedef typename OutElem<DT>::type E;
+    extern __shared__ __align__(16) uint32_t smem[];     // [32][BP]
+    const int lane = threadIdx.x & 31, u = threadIdx.x >> 5;
+    const uint64_t s0 = (uint64_t)blockIdx.x * 32;
+    const int n_live = ns - s0 < 32 ? (int)(ns - s0) : 32;
+    const bool live = lane < n_live;
+    {
+        const uint32_t smem_s = (uint32_t)__cvta_generic_to_shared(smem);
+        for (int q = u; q < n_live; q += BW) {             // warp u loads windows u, u + 8, ...
+            const uint32_t *src = st_in + (s0 + q) * NW;
+#pragma unroll 5
+            for (int k = 0; k < 20; k++) {
+                const int j = k * 32 + lane;
+                if (j < NW)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::
+                                 "r"(smem_s + (uint32_t)(q * BP + j) * 4u), "l"(src + j));
+            }
+        }
+        asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
+    }
+    __syncthreads();
+    uint32_t *A = smem + lane * BP;
+    E *rowp = out + s0 + lane;
+    uint64_t left = n;
+    if (n_live == 32) {
+        for (; left >= NW; left -= NW, rowp += (uint64_t)NW * ns)
+            mt_bround<DT, HI, false, true>(A, u, rowp, ns, true, NW, c);
+    } else {
+        for (; left >= NW; left -= NW, rowp += (uint64_t)NW * ns)
+            mt_bround<DT, HI, false, false>(A, u, rowp, ns, live, NW, c);
+    }
+    const int rem = (int)left;
+    if (rem) mt_bround<DT, HI, true, false>(A, u, rowp, ns, live, rem, c);
+    __syncthreads();
+    for (int q = u; q < n_live; q += BW) {
+        uint32_t *dst = st_out + (s0 + q) * NW;
+#pragma unroll 4
+        for (int k = 0; k < 20; k++) {
+            const int j = k * 32 + lane;
+            if (j < NW) {
+                int p = j + rem;
+                if (p >= NW) p -= NW;
+                dst[j] = smem[q * BP + p];
+            }
+        }
+    }
+}
+
+template <int DT, int HI> cudaError_t launch_bgen(cudaStream_t stream, const GenArgs &a)
+{
+    typedef typename OutElem<DT>::type E;
+    auto kern = mt19937_bgen_kernel<DT, HI>;
+    const size_t smem = (size_t)32 * BP * sizeof(uint32_t);
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    const uint64_t blocks = ceil_div_u64(a.n_streams, 32);
+    const MtMul c = {2u * 0x1908B0DFu, 1u << 31, 1u << 21, 1u << 14};
+    kern<<<(unsigned)blocks, BW * 32, smem, stream>>>((const uint32_t *)a.st_in, (uint32_t *)a.st_out, (E *)a.out,
+                                                      a.n_streams, a.n, c);
     return cudaGetLastError();
 }
 
-template <int G> cudaError_t dispatch_dt(cudaStream_t stream, const GenArgs &a)
+template <int HI> cudaError_t dispatch_bdt(cudaStream_t stream, const GenArgs &a)
 {
     switch (a.dtype) {
-    case DT_U32: return launch_gen<G, DT_U32>(stream, a);
-    case DT_F32: return launch_gen<G, DT_F32>(stream, a);
-    default: return launch_gen<G, DT_F64>(stream, a);
+    case DT_U32: return launch_bgen<DT_U32, HI>(stream, a);
+    case DT_F32: return launch_bgen<DT_F32, HI>(stream, a);
+    default: return launch_bgen<DT_F64, HI>(stream, a);
     }
 }
 
@@ -182,13 +494,17 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
 cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *li)
 {
     li->launches = 1;
-    // few streams: small CTAs so that more SMs get work; many streams: full 128-byte row segments
-    if (a.n_streams >= 32ull * 2 * (uint64_t)sm_count()) {
-        li->kernel = "mt19937_gen<G=32>";
-        return dispatch_dt<32>(stream, a);
+    // a thread's byte offset inside a row block must fit 32 bits (wave of 208 rows, 8-byte elements)
+    if (a.n_streams > ((1ull << 32) / (208 * 8)) - 8) return cudaErrorInvalidValue;
+    // Kernel choice by stream count (measured on B200): 32 streams per CTA need >= ~128
+    // CTAs; below that 8 streams per CTA; below ~1000 streams 4 per CTA in sector-sharing cluster pairs.
+    int cfg = a.n_streams >= 4096 ? 0 : a.n_streams >= 1024 ? 1 : 2;
+    if (const char *env = std::getenv("PRAND_MT_CFG")) cfg = std::atoi(env);   // test hook: force a variant
+    switch (cfg) {
+    case 0: li->kernel = "mt19937_bgen<S=32>"; return dispatch_bdt<0>(stream, a);
+    case 1: li->kernel = "mt19937_gen<S=8,T=104>"; return dispatch_dt<8, 104, 2, 6, false>(stream, a);
+    default: li->kernel = "mt19937_gen<S=4,T=208,pair>"; return dispatch_dt<4, 208, 1, 6, true>(stream, a);
     }
-    li->kernel = "mt19937_gen<G=8>";
-    return dispatch_dt<8>(stream, a);
 }
 
 }  // namespace prand

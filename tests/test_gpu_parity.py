@@ -86,6 +86,22 @@ def test_every_output_and_state_matches_oracle(gen, dtype):
         assert st == wst, f"{w.name} {gen}: exported states differ"
 
 
+@pytest.mark.parametrize("cfg", range(3))
+def test_mt19937_every_kernel_configuration(cfg, monkeypatch):
+    """Every (streams per CTA, word slices, barrier interval, pipe mix, cluster pairing) variant of
+    the MT19937 generation kernel, over whole rounds of 624, several rounds and ragged tails, with
+    stream counts that leave CTAs partly or wholly dead."""
+    need_gpu()
+    monkeypatch.setenv("PRAND_MT_CFG", str(cfg))
+    for ns, calls, dtype in [(5, [624, 1248, 1, 700], "u32"), (13, [2048], "f32"), (8, [1500, 623], "f64"), (70, [209, 1300], "u32")]:
+        w = Workload(f"mt-cfg{cfg}", "mt19937", 5489, ns, 1000, sum(calls), dtype)
+        got, st, _ = lib_run(w, calls=calls)
+        want, wst = oracle_run(w)
+        assert_same(w, got, want)
+        assert st == wst, f"cfg {cfg}: exported states differ"
+    monkeypatch.delenv("PRAND_MT_CFG")
+
+
 @pytest.mark.parametrize("gen", ALL_GENS)
 def test_successive_calls_continue_the_streams(gen):
     need_gpu()
