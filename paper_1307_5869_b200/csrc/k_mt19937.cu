@@ -141,11 +141,16 @@ __device__ __forceinline__ void cluster_wait()
 
 // One round (FULL) or the first `rem` words of one (the tail of a call).  ob = this thread's byte
 // offset (row t, stream s) from the uniform row-block pointer `rows`.
-template <int S, int T, int M, int DT, int HI, bool FULL, bool ALL>
+// In full rounds the tempering and the global store of a number are deferred until the shared loads
+// of the thread's next number have been issued: after a barrier every warp of the CTA waits for
+// shared memory at the same time, and the deferred work (half of a number's instructions, with no
+// consumer) is what fills that wait.  pend / pend_p carry the deferred number across barriers and
+// rounds; FIRST marks the call's first round, whose first step has nothing pending.
+template <int S, int T, int M, int DT, int HI, bool FULL, bool ALL, bool FIRST>
 __device__ __forceinline__ void mt_round(uint32_t *smem, const uint32_t ia, const uint32_t ib, const int t,
                                          uint32_t (&r)[NW / T], char *rows, const uint32_t ob,
                                          const uint64_t wave_bytes, const bool live, const int rem,
-                                         const MtMul &c)
+                                         const MtMul &c, uint32_t &pend, typename OutElem<DT>::type *&pend_p)
 {
     typedef typename OutElem<DT>::type E;
     constexpr int K = NW / T;
@@ -158,12 +163,22 @@ __device__ __forceinline__ void mt_round(uint32_t *smem, const uint32_t ia, cons
             if (T * (j + 1) <= NW - MW) xm = smem[ia + T * j + MW];
             else if (T * j >= NW - MW) xm = smem[ib + T * j - (NW - MW)];
             else xm = smem[(w < NW - MW ? ia + MW : ib - (NW - MW)) + T * j];
+            if (FULL && !(FIRST && j == 0)) {
+                const E v = convert<DT>(mt_temper2<HI>(pend, c));
+                if (ALL || live) store1(pend_p, v);
+            }
             const uint32_t nw = mt_recur2<HI>(r[j], x1, xm, c);
             r[j] = nw;
             smem[ib + T * j] = nw;
             if (j == 0 && t == 0) smem[ia + NW] = nw;       // x_{w+1} of word 623 is the new word 0
-            const E v = convert<DT>(mt_temper2<HI>(nw, c));
-            if (ALL || live) store1(reinterpret_cast<E *>(rows + j * wave_bytes + ob), v);
+            E *q = reinterpret_cast<E *>(rows + j * wave_bytes + ob);
+            if (FULL) {
+                pend = nw;
+                pend_p = q;
+            } else {
+                const E v = convert<DT>(mt_temper2<HI>(nw, c));
+                if (ALL || live) store1(q, v);
+            }
         }
         if ((j + 1) % M == 0) __syncthreads();
     }
@@ -206,36 +221,37 @@ mt19937_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
     uint64_t left = n;
     uint32_t cur = 0;                                     // buffer that holds the old window
     bool pending = false;
-    if (n_live == S) {
-        while (left >= NW) {
-            mt_round<S, T, M, DT, HI, true, true>(smem, ia, ib, t, r, rows, ob, wave_bytes, true, NW, c);
-            if (PAIR) {                                   // stay within one round of the sector partner
-                if (pending) cluster_wait();
-                cluster_arrive();
-                pending = true;
-            }
-            const uint32_t tmp = ia; ia = ib; ib = tmp;
-            cur ^= 1;
-            rows += round_bytes;
-            left -= NW;
-        }
-    } else {
-        while (left >= NW) {
-            mt_round<S, T, M, DT, HI, true, false>(smem, ia, ib, t, r, rows, ob, wave_bytes, live, NW, c);
-            if (PAIR) {
-                if (pending) cluster_wait();
-                cluster_arrive();
-                pending = true;
-            }
-            const uint32_t tmp = ia; ia = ib; ib = tmp;
-            cur ^= 1;
-            rows += round_bytes;
-            left -= NW;
-        }
+    uint32_t pend = 0;
+    E *pend_p = nullptr;
+#define PRAND_MT_ROUNDS(ALLV, LIVEV)                                                                         \
+    if (left >= NW) {                                                                                        \
+        mt_round<S, T, M, DT, HI, true, ALLV, true>(smem, ia, ib, t, r, rows, ob, wave_bytes, LIVEV, NW, c,  \
+                                                    pend, pend_p);                                           \
+        for (;;) {                                                                                           \
+            if (PAIR) {                                   /* stay within one round of the sector partner */ \
+                if (pending) cluster_wait();                                                                 \
+                cluster_arrive();                                                                            \
+                pending = true;                                                                              \
+            }                                                                                                \
+            const uint32_t tmp = ia; ia = ib; ib = tmp;                                                      \
+            cur ^= 1;                                                                                        \
+            rows += round_bytes;                                                                             \
+            left -= NW;                                                                                      \
+            if (left < NW) break;                                                                            \
+            mt_round<S, T, M, DT, HI, true, ALLV, false>(smem, ia, ib, t, r, rows, ob, wave_bytes, LIVEV,    \
+                                                         NW, c, pend, pend_p);                               \
+        }                                                                                                    \
+        if (ALLV || LIVEV) store1(pend_p, convert<DT>(mt_temper2<HI>(pend, c)));                             \
     }
+    if (n_live == S) {
+        PRAND_MT_ROUNDS(true, true)
+    } else {
+        PRAND_MT_ROUNDS(false, live)
+    }
+#undef PRAND_MT_ROUNDS
     if (PAIR && pending) cluster_wait();
     const int rem = (int)left;
-    if (rem) mt_round<S, T, M, DT, HI, false, false>(smem, ia, ib, t, r, rows, ob, wave_bytes, live, rem, c);
+    if (rem) mt_round<S, T, M, DT, HI, false, false, false>(smem, ia, ib, t, r, rows, ob, wave_bytes, live, rem, c, pend, pend_p);
     // final window x_{P+n}..x_{P+n+623}: words [rem, 624) of the old buffer, then [0, rem) of the new
     const uint32_t *a0 = smem + cur * (S * P), *b0 = smem + (cur ^ 1) * (S * P);
     for (int i = tid; i < S * NW; i += NT) {
@@ -502,7 +518,7 @@ cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *
     if (const char *env = std::getenv("PRAND_MT_CFG")) cfg = std::atoi(env);   // test hook: force a variant
     switch (cfg) {
     case 0: li->kernel = "mt19937_bgen<S=32>"; return dispatch_bdt<0>(stream, a);
-    case 1: li->kernel = "mt19937_gen<S=8,T=104>"; return dispatch_dt<8, 104, 2, 6, false>(stream, a);
+    case 1: li->kernel = "mt19937_gen<S=8,T=104>"; return dispatch_dt<8, 104, 2, 0, false>(stream, a);
     default: li->kernel = "mt19937_gen<S=4,T=208,pair>"; return dispatch_dt<4, 208, 1, 6, true>(stream, a);
     }
 }
