@@ -58,6 +58,7 @@ struct GenArgs {
     uint64_t chunk_len;
     uint64_t n_chunks;
     const void *chunk_ops;
+    bool clean;            // GM55/GQ58: every state word is a multiple of 2^t (see k_gmgq.cu)
 };
 
 struct LaunchInfo { const char *kernel; unsigned launches; };

@@ -149,6 +149,8 @@ struct prand_state {
     bool host_ready;
     const char *last_kernel;
     cudaStream_t last_stream;   // stream of the most recent call: prand_free releases in its order
+    bool gm_clean;          // GM55/GQ58: every state word is a multiple of 2^t (true for states the
+                            // library creates; an imported state is scanned), see k_gmgq.cu
 };
 
 namespace {
@@ -357,6 +359,7 @@ extern "C" int prand_init_shard(prand_state **out, int gen, uint64_t seed, uint6
         if (rc) return rc;
     }
     prand_state *st = new (std::nothrow) prand_state();
+    if (st) st->gm_clean = true;
     if (!st) return PRAND_ERR_ALLOC;
     std::memset(st, 0, sizeof *st);
     st->gen = gen;
@@ -418,6 +421,7 @@ extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_l
         CU(launch_jump(stream, st->gen, a, &li));
     }
     note(st, li);
+    if (steps_log2 >= 4 || steps_mant >= 16) st->gm_clean = true;   // past the 2-adic transient
     return PRAND_OK;
 }
 
@@ -445,10 +449,7 @@ void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t 
         uint64_t per_thread_streams = 1, lanes_per_stream = 1, min_len = 64;
         if (gen == PRAND_LFSR113) per_thread_streams = 4;
         else if (gen == PRAND_MRG32K3A) per_thread_streams = dtype == DT_F64 ? 2 : 4;
-        else {
-            min_len = 128;
-            if (gen == PRAND_GM61 || gen == PRAND_GQ58_1) lanes_per_stream = 4;
-        }
+        else min_len = 128;
         uint64_t threads = ns * lanes_per_stream / per_thread_streams;
         if (threads == 0) threads = 1;
         // one balanced wave: as many equal chunks as fit the threads resident at once, never more
@@ -506,6 +507,7 @@ int generate(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t str
     a.n = n;
     plan_chunks(st->gen, st->ns, n, dtype, sm_count(), &a.chunk_len, &a.n_chunks);
     a.chunk_ops = nullptr;
+    a.clean = st->gm_clean;
     a.st_in = st->d_state[st->cur];
     a.st_out = st->d_state[st->cur];
     if (a.n_chunks > 1) {
@@ -526,6 +528,7 @@ int generate(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t str
     if (e != cudaSuccess) return cuda_fail(e);
     note(st, li);
     if (a.n_chunks > 1) st->cur = 1 - st->cur;
+    if (n >= 16) st->gm_clean = true;
     return PRAND_OK;
 }
 
@@ -668,6 +671,16 @@ extern "C" int prand_set_state(prand_state *st, const void *host_buf, size_t byt
         return PRAND_OK;
     }
     std::vector<unsigned char> tmp(bytes);
+    if (const GmParams *gp = gm_params(st->gen)) {
+        // GM55/GQ58 (g = 2^t p): the fast kernels need every word to be a multiple of 2^t
+        st->gm_clean = true;
+        const uint64_t odd_g = gp->g & (0 - gp->g);          // 2^t
+        if (odd_g > 1 && gp->wide) {
+            const uint64_t *w = (const uint64_t *)host_buf;
+            for (size_t i = 0; i < st->ns * words && st->gm_clean; i++)
+                if (w[i] & (odd_g - 1)) st->gm_clean = false;
+        }
+    }
     if (state_word_bytes(st->gen) == 8) canon_to_soa((const uint64_t *)host_buf, (uint64_t *)tmp.data(), st->ns, words);
     else canon_to_soa((const uint32_t *)host_buf, (uint32_t *)tmp.data(), st->ns, words);
     CU(cudaMemcpy(st->d_state[st->cur], tmp.data(), bytes, cudaMemcpyHostToDevice));

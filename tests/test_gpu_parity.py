@@ -173,6 +173,40 @@ def test_state_roundtrip_through_the_host(gen):
     a.close(); b.close()
 
 
+@pytest.mark.parametrize("gen", ["gm55", "gq58.1", "gq58.3", "gq58.4"])
+def test_imported_states_inside_the_two_adic_transient(gen):
+    """g = 2^t p: the library's own states are multiples of 2^t and run the mod-p kernels; an imported
+    state need not be (any residue mod g is a state).  Such states take the plain mod-g kernels until
+    they have advanced 16 steps; outputs and states must equal the oracle's throughout."""
+    need_gpu()
+    ns = 9
+    g_mod = {"gm55": 16 * (2**51 - 129)}.get(gen, 2**29 * (2**29 - 3))
+    s_pts = {"gm55": 8, "gq58.1": 32, "gq58.3": 12, "gq58.4": 8}[gen]
+    rng = np.random.default_rng(7)
+    words = rng.integers(0, g_mod, size=(ns, 2 * s_pts), dtype=np.uint64)
+    words[0, :] = [1, 0] * s_pts                           # degenerate small values too
+    words[1, :] = g_mod - 1
+    blob = words.tobytes()
+    g = P.Generator(gen, 1, ns, 0)
+    g.set_state(blob)
+    calls = [3, 5, 9, 40, 25]
+    got = []
+    for n in calls:
+        got.append(g.generate(n, "u32").cpu().numpy().view(np.uint32))
+        if n == 9:
+            assert "plain" in g.last_kernel
+    assert "plain" not in g.last_kernel                   # past the transient: the mod-p kernel
+    got = np.concatenate(got, 0)
+    st = g.state()
+    g.close()
+    per = 2 * s_pts * 8
+    for s in range(ns):
+        o = oracle.State(gen, 1).load(blob[s * per:(s + 1) * per])
+        want = o.fill(sum(calls), "u32")
+        assert np.array_equal(got[:, s], want), f"{gen}: stream {s} differs from the oracle"
+        assert st[s * per:(s + 1) * per] == o.export()
+
+
 @pytest.mark.parametrize("gen,dtype", [("lfsr113", "u32"), ("mrg32k3a", "f64"), ("gm31", "f32"), ("mt19937", "u32")])
 def test_host_delivery_equals_device_fill(gen, dtype):
     """rng_generate_array_: same numbers, delivered to host memory."""
