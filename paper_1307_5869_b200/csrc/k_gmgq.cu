@@ -89,15 +89,10 @@ template <> struct Gm<PRAND_GM31> {
     __device__ static __forceinline__ W store(R x) { return x; }
     __device__ static __forceinline__ R step(R xP, R xN)
     {
-        // t = 11 xN - 14 xP + 14 g in (0, 25 * 2^31): one unsigned and one signed 32x32+64 multiply-add,
-        // the constant riding as the addend of the first
-        uint64_t t;
-        asm("{\n\t.reg .u64 k;\n\t"
-            "mov.u64 k, 0x6FFFFFFF2;\n\t"                 // 14 g
-            "mad.wide.u32 %0, %1, 11, k;\n\t"
-            "mad.wide.s32 %0, %2, -14, %0;\n\t}"
-            : "=l"(t) : "r"(xN), "r"(xP));
-        uint32_t h = (uint32_t)((uint64_t)t >> 31);        // < 25
+        // t = 11 xN + 14 (g - xP) < 25 * 2^31: g - xP = xP ^ g (g is all ones), two chained 32x32+64
+        // multiply-adds (a 64-bit constant addend would cost two more adds)
+        const uint64_t t = (uint64_t)(xP ^ G) * 14u + (uint64_t)xN * 11u;
+        uint32_t h = (uint32_t)(t >> 31);                  // < 25
         uint32_t r = h * 0x80000001u + (uint32_t)t;        // lo - h 2^31 + h = (t & g) + (t >> 31) < 2^31 + 25
         return umin_sub(r, G);
     }
