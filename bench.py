@@ -51,12 +51,17 @@ def load_peaks():
 
 
 def load_traffic(kernel: str):
-    """dram bytes per launch of `kernel` from the committed ncu --set full capture, or None."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed
+    ncu --set full capture (profiles/traffic.csv names the details file it came from), or None."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(path):
         return None
-    with open(path) as f:
-        return json.load(f).get(kernel)
+    import csv
+    with open(path, newline="") as f:
+        for row in csv.DictReader(f):
+            if row["kernel"] == kernel:
+                return int(row["dram_bytes_per_launch"])
+    return None
 
 
 class ClockSampler:

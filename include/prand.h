@@ -124,6 +124,21 @@ int prand_generate_f32_host(prand_state *st, float *host_out, uint64_t n_per_str
 int prand_generate_f64_host(prand_state *st, double *host_out, uint64_t n_per_stream, void *cuda_stream);
 
 /*
+ * prand_generate_seq_{u32,f32,f64} -- PRAND's single-sequence array fill ("the output
+ *   array is divided into sections ... jumping ahead to a starting point of the section", Table 5
+ *   PAPER.md:384-404, rng_generate_gpu_array_ PAPER.md:465).  `st` must hold exactly one stream
+ *   (n_streams == 1, else PRAND_ERR_ARG).  out[j], j < length, = output number j of that stream counted
+ *   from its current position, i.e. exactly what `length` successive single-stream generate calls
+ *   would have produced; afterwards the stream has advanced by `length`.  `out` is caller-owned DEVICE
+ *   memory with `length` elements.  Unlike PRAND no divisibility of `length` by the
+ *   number of sections is required (MT19937: no power of two).  The library allocates
+ *   (stream-ordered) a scratch buffer of about `length` elements for the duration of the call.
+ */
+int prand_generate_seq_u32(prand_state *st, uint32_t *out, uint64_t length, void *cuda_stream);
+int prand_generate_seq_f32(prand_state *st, float *out, uint64_t length, void *cuda_stream);
+int prand_generate_seq_f64(prand_state *st, double *out, uint64_t length, void *cuda_stream);
+
+/*
  * Canonical state export / import (the state is plain data and may be copied between
  * host and device; generation continues from it).  Per stream, little-endian, streams consecutive:
  *   LFSR113   4 x u32  z1..z4 masked to their significant top 31/29/28/25 bits;

@@ -37,6 +37,9 @@ _SIGS = {
     "prand_set_state": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "prand_n_streams": (C.c_uint64, [C.c_void_p]),
     "prand_gen_of": (C.c_int, [C.c_void_p]),
+    "prand_generate_seq_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_generate_seq_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_generate_seq_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_free": (C.c_int, [C.c_void_p]),
     "prand_fill_u32": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p]),
     "prand_launch_count": (C.c_uint64, []),
@@ -253,6 +256,17 @@ class Generator:
             assert out.is_cuda and out.is_contiguous() and out.dtype == tdt
             assert out.numel() == n_per_stream * self.n_streams
         _generate("prand_generate_" + dtype, self._h, out.data_ptr(), n_per_stream, stream)
+        return out
+
+    def generate_seq(self, length: int, dtype: str = "u32", out=None, stream=None):
+        """PRAND's single-sequence fill (n_streams must be 1): the next ``length`` numbers, in order."""
+        import torch
+        tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
+        if out is None:
+            out = torch.empty(length, dtype=tdt, device="cuda")
+        else:
+            assert out.is_cuda and out.is_contiguous() and out.dtype == tdt and out.numel() == length
+        _generate("prand_generate_seq_" + dtype, self._h, out.data_ptr(), length, stream)
         return out
 
     def generate_host(self, n_per_stream: int, dtype: str = "u32", out=None, stream=None):

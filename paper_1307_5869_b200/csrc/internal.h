@@ -75,6 +75,9 @@ cudaError_t mt19937_apply(cudaStream_t, const uint32_t *st_src, uint32_t *st_dst
                           uint64_t count, uint64_t src_back, const MtOp *d_op, LaunchInfo *);
 cudaError_t mt19937_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
 cudaError_t fill_u32(cudaStream_t, uint32_t *out, uint64_t n_words, uint32_t value, LaunchInfo *);
+// out[c * sec_len + i] = tmp[i * n_sections + c] for c * sec_len + i < length (elem_bytes 4 or 8)
+cudaError_t transpose_sections(cudaStream_t, const void *tmp, void *out, uint64_t n_sections, uint64_t sec_len,
+                               uint64_t length, int elem_bytes, LaunchInfo *);
 
 int sm_count();   // cached multiprocessor count of the current device
 

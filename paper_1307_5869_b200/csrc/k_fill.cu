@@ -16,7 +16,45 @@ fill_u32_kernel(uint32_t *__restrict__ out, uint64_t n_vec, uint64_t n_words, ui
     if (blockIdx.x == 0 && threadIdx.x < (n_words & 3)) out[n_vec * 4 + threadIdx.x] = value;
 }
 
+// Sections of a single sequence (prand_generate_seq_*): the bulk kernels fill the family of sections
+// in the interleaved layout tmp[i * S + c]; PRAND's array layout is out[c * L + i].
+// 32 x 32 tiles through shared memory, both sides coalesced.
+template <class E>
+__global__ void __launch_bounds__(256)
+transpose_sections_kernel(const E *__restrict__ tmp, E *__restrict__ out, uint64_t S, uint64_t L, uint64_t length)
+{
+    __shared__ E tile[32][33];
+    const uint64_t i0 = (uint64_t)blockIdx.x * 32, c0 = (uint64_t)blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const uint64_t i = i0 + r, c = c0 + tx;
+        if (i < L && c < S) tile[r][tx] = tmp[i * S + c];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const uint64_t c = c0 + r, i = i0 + tx;
+        if (c < S && i < L && c * L + i < length) __stcs(out + c * L + i, tile[tx][r]);
+    }
+}
+
 }  // namespace
+
+cudaError_t transpose_sections(cudaStream_t stream, const void *tmp, void *out, uint64_t n_sections,
+                               uint64_t sec_len, uint64_t length, int elem_bytes, LaunchInfo *li)
+{
+    dim3 grid((unsigned)ceil_div_u64(sec_len, 32), (unsigned)ceil_div_u64(n_sections, 32));
+    if (elem_bytes == 8)
+        transpose_sections_kernel<uint64_t><<<grid, 256, 0, stream>>>((const uint64_t *)tmp, (uint64_t *)out,
+                                                                      n_sections, sec_len, length);
+    else
+        transpose_sections_kernel<uint32_t><<<grid, 256, 0, stream>>>((const uint32_t *)tmp, (uint32_t *)out,
+                                                                      n_sections, sec_len, length);
+    li->kernel = "transpose_sections";
+    li->launches = 1;
+    return cudaGetLastError();
+}
 
 cudaError_t fill_u32(cudaStream_t stream, uint32_t *out, uint64_t n_words, uint32_t value, LaunchInfo *li)
 {

@@ -149,6 +149,7 @@ struct prand_state {
     bool host_ready;
     const char *last_kernel;
     cudaStream_t last_stream;   // stream of the most recent call: prand_free releases in its order
+    prand_state *sec;       // prand_generate_seq_*: cached family of sections (one stream per section)
     bool gm_clean;          // GM55/GQ58: every state word is a multiple of 2^t (true for states the
                             // library creates; an imported state is scanned), see k_gmgq.cu
 };
@@ -249,12 +250,13 @@ namespace {
 
 // MT19937: stream 0 of the shard = seed window jumped first * L; then a doubling tree -- level j
 // fills local streams [2^j, 2^(j+1)) from [0, 2^j) with g_{L 2^j} (eq. 10), one application each.
-int init_mt19937(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
+// d_base != nullptr: the family starts from that device-resident one-stream state instead of the seed.
+int init_mt19937(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream, const void *d_base = nullptr)
 {
     const unsigned lev_all = bit_length(st->first + st->ns - 1);
     const unsigned lev_tree = bit_length(st->ns - 1);
     std::vector<unsigned char> base;
-    int rc = build_seed_state(PRAND_MT19937, seed, base);
+    int rc = d_base ? PRAND_OK : build_seed_state(PRAND_MT19937, seed, base);
     if (rc) return rc;
     std::vector<host::MtPoly> polys;
     host::mt19937_levels(L, lev_all, polys);
@@ -274,7 +276,8 @@ int init_mt19937(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
     if (rc) return rc;
     UPLOAD(st->d_ops, ops.data(), ops.size() * sizeof(MtOp), stream);
     uint32_t *d = (uint32_t *)st->d_state[st->cur];
-    UPLOAD(d, base.data(), base.size(), stream);
+    if (d_base) { CU(cudaMemcpyAsync(d, d_base, stream_bytes(PRAND_MT19937), cudaMemcpyDeviceToDevice, stream)); }
+    else UPLOAD(d, base.data(), base.size(), stream);
     const MtOp *d_ops = (const MtOp *)st->d_ops;
     LaunchInfo li;
     if (have_first) {
@@ -290,19 +293,21 @@ int init_mt19937(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
     return PRAND_OK;
 }
 
-int init_body(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream)
+int init_body(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream, const void *d_base = nullptr)
 {
-    if (st->gen == PRAND_MT19937) return init_mt19937(st, seed, L, stream);
+    if (st->gen == PRAND_MT19937) return init_mt19937(st, seed, L, stream, d_base);
     std::vector<unsigned char> base, ops;
-    int rc = build_seed_state(st->gen, seed, base);
+    int rc = d_base ? PRAND_OK : build_seed_state(st->gen, seed, base);
     if (rc) return rc;
+    if (d_base) base.assign(stream_bytes(st->gen), 0);
     const unsigned levels = bit_length(st->first + st->ns - 1);
     rc = build_level_ops(st->gen, L, levels, ops);
     if (rc) return rc;
     const size_t ops_off = (base.size() + 255) & ~(size_t)255;
     rc = ensure_ops(st, ops_off + ops.size() + 256);
     if (rc) return rc;
-    UPLOAD(st->d_ops, base.data(), base.size(), stream);
+    if (d_base) { CU(cudaMemcpyAsync(st->d_ops, d_base, base.size(), cudaMemcpyDeviceToDevice, stream)); }
+    else UPLOAD(st->d_ops, base.data(), base.size(), stream);
     if (!ops.empty())
         UPLOAD((char *)st->d_ops + ops_off, ops.data(), ops.size(), stream);
     JumpArgs a;
@@ -333,6 +338,7 @@ void destroy(prand_state *st)
     if (st->host_ready) cudaStreamDestroy(st->copy_stream);
     if (st->d_ops) cudaFreeAsync(st->d_ops, s);
     if (st->d_chunk_ops) cudaFreeAsync(st->d_chunk_ops, s);
+    if (st->sec) { st->sec->last_stream = s; destroy(st->sec); }
     delete st;
 }
 
@@ -359,9 +365,9 @@ extern "C" int prand_init_shard(prand_state **out, int gen, uint64_t seed, uint6
         if (rc) return rc;
     }
     prand_state *st = new (std::nothrow) prand_state();
-    if (st) st->gm_clean = true;
     if (!st) return PRAND_ERR_ALLOC;
     std::memset(st, 0, sizeof *st);
+    st->gm_clean = true;
     st->gen = gen;
     st->ns = n_streams;
     st->first = first_stream;
@@ -610,6 +616,93 @@ extern "C" int prand_generate_f32_host(prand_state *st, float *out, uint64_t n, 
 extern "C" int prand_generate_f64_host(prand_state *st, double *out, uint64_t n, void *s)
 {
     return generate_host(st, out, n, DT_F64, (cudaStream_t)s);
+}
+
+// ==================================================================================================
+// prand_generate_seq_* (SURVEY.md 8(f)1): PRAND's single-sequence array fill
+// ==================================================================================================
+namespace {
+
+// PAPER.md:382, Table 5: the array is divided into sections, each section is
+// reached by jump-ahead and filled in parallel; the result is what the serial generator would have
+// produced.  Here: section c = a stream that starts c * sec_len ahead of the state, the family is
+// filled in the interleaved layout by the bulk kernels and transposed into out[c * sec_len + i].
+void plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec_len)
+{
+    // enough sections to fill the GPU, sections long enough to amortise the jump to their start
+    const uint64_t min_len = gen == PRAND_MT19937 ? 8 * 624 : 1024;
+    const uint64_t max_sec = gen == PRAND_MT19937 ? 4096 : 65536;
+    uint64_t S = length / min_len;
+    if (S > max_sec) S = max_sec;
+    if (S < 1) S = 1;
+    uint64_t L = (length + S - 1) / S;
+    L = (L + 31) / 32 * 32;
+    *sec_len = L;
+    *n_sections = (length + L - 1) / L;
+}
+
+int generate_seq(prand_state *st, void *out, uint64_t length, int dtype, cudaStream_t stream)
+{
+    if (!st || (!out && length)) return PRAND_ERR_ARG;
+    if (st->ns != 1) return PRAND_ERR_ARG;                 // one sequence: the state of a single stream
+    if (length == 0) return PRAND_OK;
+    uint64_t S, L;
+    plan_sections(st->gen, length, &S, &L);
+    if (S == 1) return generate(st, out, length, dtype, stream);
+    st->last_stream = stream;
+    const size_t esz = dtype == DT_F64 ? 8 : 4;
+    if ((uintptr_t)out % esz) return PRAND_ERR_ARG;
+    // the family of sections (cached across calls of the same shape)
+    if (st->sec && st->sec->ns != S) { st->sec->last_stream = stream; destroy(st->sec); st->sec = nullptr; }
+    if (!st->sec) {
+        prand_state *c = new (std::nothrow) prand_state();
+        if (!c) return PRAND_ERR_ALLOC;
+        std::memset(c, 0, sizeof *c);
+        c->gen = st->gen;
+        c->ns = S;
+        c->bytes = (size_t)S * stream_bytes(st->gen);
+        c->last_kernel = "";
+        c->last_stream = stream;
+        c->device = st->device;
+        cudaError_t e = dev_alloc(&c->d_state[0], c->bytes, stream);
+        if (e != cudaSuccess) { delete c; return cuda_fail(e); }
+        st->sec = c;
+    }
+    prand_state *c = st->sec;
+    c->cur = 0;
+    c->gm_clean = st->gm_clean;
+    c->last_stream = stream;
+    Dist Ld = {L, 0};
+    int rc = init_body(c, 0, Ld, stream, st->d_state[st->cur]);
+    if (rc) return rc;
+    void *tmp = nullptr;
+    CU(dev_alloc(&tmp, (size_t)L * S * esz, stream));
+    rc = generate(c, tmp, L, dtype, stream);
+    if (rc == PRAND_OK) {
+        LaunchInfo li;
+        cudaError_t e = transpose_sections(stream, tmp, out, S, L, length, (int)esz, &li);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+        else note(st, li);
+        st->last_kernel = c->last_kernel;
+    }
+    CU(cudaFreeAsync(tmp, stream));
+    if (rc) return rc;
+    return prand_jump(st, length, 0, stream);              // the sequence has advanced by `length`
+}
+
+}  // namespace
+
+extern "C" int prand_generate_seq_u32(prand_state *st, uint32_t *out, uint64_t length, void *s)
+{
+    return generate_seq(st, out, length, DT_U32, (cudaStream_t)s);
+}
+extern "C" int prand_generate_seq_f32(prand_state *st, float *out, uint64_t length, void *s)
+{
+    return generate_seq(st, out, length, DT_F32, (cudaStream_t)s);
+}
+extern "C" int prand_generate_seq_f64(prand_state *st, double *out, uint64_t length, void *s)
+{
+    return generate_seq(st, out, length, DT_F64, (cudaStream_t)s);
 }
 
 // ==================================================================================================

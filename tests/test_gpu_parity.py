@@ -224,6 +224,37 @@ def test_host_delivery_equals_device_fill(gen, dtype):
     g.close(); g2.close()
 
 
+@pytest.mark.parametrize("gen", ALL_GENS)
+def test_single_sequence_fill_equals_the_serial_generator(gen):
+    """PAPER.md:382, 402-404 (rng_generate_gpu_array_): the array is cut into sections reached by
+    jump-ahead, and holds exactly the numbers the serial generator produces, for any length."""
+    need_gpu()
+    seed = workloads.SEED.get(gen, 1)
+    lengths = [100000, 7, 40001] if gen != "mt19937" else [30000, 5, 12345]
+    for dtype in (["u32", "f64"] if gen in ("mrg32k3a", "gm31") else ["u32"]):
+        g = P.Generator(gen, seed, 1, 0)
+        g.jump(3)
+        got = [g.generate_seq(n, dtype).cpu().numpy().view(NPDT[dtype]) for n in lengths]
+        tail = g.generate(9, dtype).cpu().numpy().view(NPDT[dtype])[:, 0]     # the stream has advanced
+        if lengths[0] >= 8 * 1024:
+            assert "transpose" not in g.last_kernel
+        st = g.state()
+        g.close()
+        o = oracle.State(gen, seed).jump(3)
+        want = o.fill(sum(lengths) + 9, dtype)
+        gotall = np.concatenate(got + [tail])
+        assert np.array_equal(gotall.view(BITS[dtype]), want.view(BITS[dtype])), f"{gen}/{dtype}"
+        assert st == o.export()
+
+
+def test_single_sequence_fill_needs_one_stream():
+    need_gpu()
+    g = P.Generator("lfsr113", 12345, 2, 1000)
+    buf = torch.empty(16, dtype=torch.int32, device="cuda")
+    assert P.lib().prand_generate_seq_u32(g._h, buf.data_ptr(), 16, None) == -2
+    g.close()
+
+
 def got_dtype(dtype):
     return {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
 
