@@ -42,6 +42,22 @@ UNIT = "Gnumbers/s"
 ARITH = {"lfsr113": "u32", "mrg32k3a": "u32 (32x32->64 mul, mod 2^32-c) + f64 scale", "mt19937": "u32"}
 
 
+# Integer-bound generators (DESIGN.md 6.4/6.5): thread-instructions per number of the generation loop
+# (SASS counts of the committed kernels, confirmed by ncu smsp__inst_executed in profiles/r01b_summary.md)
+# against the issue peak 148 SMs x 4 schedulers x 32 lanes x sm_max_mhz.
+ALU_INSTR_PER_NUMBER = {"gm19": 250, "gm29": 294, "gm31": 266, "gm61": 549, "gm55": 241, "gq58.1": 306,
+                        "gq58.3": 147, "gq58.4": 118}
+
+
+def alu_peak_ginstr():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    mhz = 1965.0
+    if os.path.exists(path):
+        with open(path) as f:
+            mhz = float(json.load(f).get("sm_max_mhz", mhz))
+    return 148 * 4 * 32 * mhz * 1e6 / 1e9
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -298,16 +314,26 @@ def run_ours(args, w):
     k_ms = statistics.mean(kernel_ms)
     achieved = w.out_bytes / (k_ms * 1e-3) / 1e9
     traffic = load_traffic(last_kernel[0])
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": traffic, "kernel": last_kernel[0], "kernel_ms": k_ms,
+                "kernel_share_of_step": k_ms / ms_per_step,
+                "algorithmic_bytes_per_launch": w.out_bytes, "peak_source": peak_src,
+                "write_peak_same_run_gbs": fill_gbs, "frac_of_write_peak": achieved / fill_gbs}
+    if w.gen in ALU_INSTR_PER_NUMBER:              # integer-bound: report against the issue peak
+        ipn = ALU_INSTR_PER_NUMBER[w.gen]
+        a_g = ipn * w.numbers / (k_ms * 1e-3) / 1e9
+        p_g = alu_peak_ginstr()
+        roofline = {"bound": "alu", "achieved": a_g, "peak": p_g, "unit": "Gthread-instr/s", "frac": a_g / p_g,
+                    "traffic": traffic, "kernel": last_kernel[0], "kernel_ms": k_ms,
+                    "kernel_share_of_step": k_ms / ms_per_step, "thread_instr_per_number": ipn,
+                    "peak_source": "148 SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md 6.5)",
+                    "out_gbs": achieved, "hbm_peak_gbs": peak}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": ARITH.get(w.gen, "u32/u64 modular"), "data": "synthetic",
         "config": config_of(w),
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic, "kernel": last_kernel[0], "kernel_ms": k_ms,
-                     "kernel_share_of_step": k_ms / ms_per_step,
-                     "algorithmic_bytes_per_launch": w.out_bytes, "peak_source": peak_src,
-                     "write_peak_same_run_gbs": fill_gbs, "frac_of_write_peak": achieved / fill_gbs},
+        "roofline": roofline,
         "e2e": e2e, "gpu_launches": launches, "clocks": clk.summary(),
     }
     if world == 1 and not args.no_cpu:

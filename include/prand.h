@@ -139,6 +139,21 @@ int prand_generate_seq_f32(prand_state *st, float *out, uint64_t length, void *c
 int prand_generate_seq_f64(prand_state *st, double *out, uint64_t length, void *cuda_stream);
 
 /*
+ * Device-callable API (the generators can be called from a user's kernel).
+ * include/prand_device.cuh holds the header-only __device__ generators; these calls give a kernel
+ * access to the library's device-resident state (layout documented in that header; the pointer stays
+ * valid until the next prand_generate_* call that uses sub-sections, prand_set_state or prand_free)
+ * and run the library's own example kernel written against that header: one thread per stream,
+ * out[i * n_streams + s] as for prand_generate_*, the streams advance by n_per_stream.  The example
+ * is a self-test of the header, not a fast path.
+ */
+void *prand_state_device_ptr(prand_state *st);
+uint64_t prand_state_n_streams(const prand_state *st);
+int prand_device_api_fill_u32(prand_state *st, uint32_t *out, uint64_t n_per_stream, void *cuda_stream);
+int prand_device_api_fill_f32(prand_state *st, float *out, uint64_t n_per_stream, void *cuda_stream);
+int prand_device_api_fill_f64(prand_state *st, double *out, uint64_t n_per_stream, void *cuda_stream);
+
+/*
  * Canonical state export / import (the state is plain data and may be copied between
  * host and device; generation continues from it).  Per stream, little-endian, streams consecutive:
  *   LFSR113   4 x u32  z1..z4 masked to their significant top 31/29/28/25 bits;

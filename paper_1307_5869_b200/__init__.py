@@ -40,6 +40,11 @@ _SIGS = {
     "prand_generate_seq_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_generate_seq_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_generate_seq_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_state_device_ptr": (C.c_void_p, [C.c_void_p]),
+    "prand_state_n_streams": (C.c_uint64, [C.c_void_p]),
+    "prand_device_api_fill_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_device_api_fill_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_device_api_fill_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_free": (C.c_int, [C.c_void_p]),
     "prand_fill_u32": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p]),
     "prand_launch_count": (C.c_uint64, []),
@@ -256,6 +261,14 @@ class Generator:
             assert out.is_cuda and out.is_contiguous() and out.dtype == tdt
             assert out.numel() == n_per_stream * self.n_streams
         _generate("prand_generate_" + dtype, self._h, out.data_ptr(), n_per_stream, stream)
+        return out
+
+    def device_api_fill(self, n_per_stream: int, dtype: str = "u32", stream=None):
+        """The library's example kernel written against include/prand_device.cuh (one thread per stream)."""
+        import torch
+        tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
+        out = torch.empty((n_per_stream, self.n_streams), dtype=tdt, device="cuda")
+        _generate("prand_device_api_fill_" + dtype, self._h, out.data_ptr(), n_per_stream, stream)
         return out
 
     def generate_seq(self, length: int, dtype: str = "u32", out=None, stream=None):

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libprand.so")
 SOURCES = ["prand.cu", "skip_ops.cpp", "k_lfsr113.cu", "k_mrg32k3a.cu", "k_mt19937.cu", "k_gmgq.cu",
-           "k_fill.cu"]
+           "k_fill.cu", "k_devapi.cu"]
 HEADERS = ["internal.h", "k_common.cuh", "skip_ops.h"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -29,7 +29,8 @@ def _stale(target: str, deps: list[str]) -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     hdrs = [os.path.join(CSRC, h) for h in HEADERS]
-    hdrs += [os.path.join(HERE, "..", "include", h) for h in ("prand.h", "prand_host.h")]
+    hdrs += [os.path.join(HERE, "..", "include", h)
+             for h in ("prand.h", "prand_host.h", "prand_device.cuh", "prand_device_gm.cuh")]
     hdrs.append(os.path.abspath(__file__))
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)

@@ -79,6 +79,10 @@ cudaError_t fill_u32(cudaStream_t, uint32_t *out, uint64_t n_words, uint32_t val
 cudaError_t transpose_sections(cudaStream_t, const void *tmp, void *out, uint64_t n_sections, uint64_t sec_len,
                                uint64_t length, int elem_bytes, LaunchInfo *);
 
+// one thread per stream through include/prand_device.cuh (example / self-test of the device API)
+cudaError_t devapi_generate(cudaStream_t, int gen, void *state, void *out, uint64_t ns, uint64_t n, int dtype,
+                            LaunchInfo *);
+
 int sm_count();   // cached multiprocessor count of the current device
 
 }  // namespace prand

@@ -706,6 +706,42 @@ extern "C" int prand_generate_seq_f64(prand_state *st, double *out, uint64_t len
 }
 
 // ==================================================================================================
+// device-callable API support
+// ==================================================================================================
+extern "C" void *prand_state_device_ptr(prand_state *st)
+{
+    return st ? st->d_state[st->cur] : nullptr;
+}
+extern "C" uint64_t prand_state_n_streams(const prand_state *st) { return st ? st->ns : 0; }
+
+namespace {
+int devapi_fill(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t stream)
+{
+    if (!st || (!out && n)) return PRAND_ERR_ARG;
+    if (n == 0) return PRAND_OK;
+    st->last_stream = stream;
+    LaunchInfo li = {"", 0};
+    cudaError_t e = devapi_generate(stream, st->gen, st->d_state[st->cur], out, st->ns, n, dtype, &li);
+    if (e != cudaSuccess) return cuda_fail(e);
+    note(st, li);
+    if (n >= 16) st->gm_clean = true;
+    return PRAND_OK;
+}
+}  // namespace
+extern "C" int prand_device_api_fill_u32(prand_state *st, uint32_t *out, uint64_t n, void *s)
+{
+    return devapi_fill(st, out, n, DT_U32, (cudaStream_t)s);
+}
+extern "C" int prand_device_api_fill_f32(prand_state *st, float *out, uint64_t n, void *s)
+{
+    return devapi_fill(st, out, n, DT_F32, (cudaStream_t)s);
+}
+extern "C" int prand_device_api_fill_f64(prand_state *st, double *out, uint64_t n, void *s)
+{
+    return devapi_fill(st, out, n, DT_F64, (cudaStream_t)s);
+}
+
+// ==================================================================================================
 // canonical state export / import
 // ==================================================================================================
 namespace {

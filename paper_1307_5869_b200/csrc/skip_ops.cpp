@@ -340,12 +340,33 @@ void mt19937_xpow(Dist n, MtPoly &out)
     out = acc;
 }
 
+// PRAND ships its jump polynomials precomputed because each costs milliseconds of serial host work
+// (PAPER.md:378).  Here they are computed on demand and the ladder x^(n 2^j) mod phi of the most
+// recent distances is kept, so that a second prand_init / prand_jump with the same distance (a
+// bench step, a family of shards) costs a copy.
 void mt19937_levels(Dist n, unsigned levels, std::vector<MtPoly> &out)
 {
+    struct Entry { Dist n; std::vector<MtPoly> ladder; };
+    static std::mutex mu;
+    static std::vector<Entry> cache;                       // most recently used last, at most 8 distances
     out.assign(levels, MtPoly());
     if (!levels) return;
-    mt19937_xpow(n, out[0]);
-    for (unsigned lev = 1; lev < levels; lev++) mt19937_sqrmod(out[lev], out[lev - 1]);
+    std::lock_guard<std::mutex> lock(mu);
+    size_t hit = cache.size();
+    for (size_t i = 0; i < cache.size(); i++)
+        if (cache[i].n.mant == n.mant && cache[i].n.log2 == n.log2) hit = i;
+    if (hit == cache.size()) {
+        if (cache.size() == 8) cache.erase(cache.begin());
+        cache.push_back(Entry{n, std::vector<MtPoly>(1)});
+        mt19937_xpow(n, cache.back().ladder[0]);
+        hit = cache.size() - 1;
+    }
+    std::vector<MtPoly> &lad = cache[hit].ladder;
+    while (lad.size() < levels) {
+        lad.emplace_back();
+        mt19937_sqrmod(lad[lad.size() - 1], lad[lad.size() - 2]);
+    }
+    for (unsigned lev = 0; lev < levels; lev++) out[lev] = lad[lev];
 }
 
 void mt19937_to_op(const MtPoly &p, MtOp &op)

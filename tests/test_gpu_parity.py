@@ -255,6 +255,28 @@ def test_single_sequence_fill_needs_one_stream():
     g.close()
 
 
+@pytest.mark.parametrize("gen", ALL_GENS)
+def test_device_callable_api_matches_oracle_and_bulk_kernels(gen):
+    """the generators are callable from a user's kernel on the library's state.
+    The library's example kernel (include/prand_device.cuh, one thread per stream) must produce the
+    oracle's numbers, leave the oracle's state, and interleave freely with the bulk kernels."""
+    need_gpu()
+    seed = workloads.SEED.get(gen, 1)
+    ns, L = (5, 1000) if gen == "mt19937" else (70, workloads.BLOCK_LEN[gen])
+    for dtype in ("u32", "f32", "f64"):
+        g = P.Generator(gen, seed, ns, L)
+        a = g.device_api_fill(21, dtype).cpu().numpy().view(NPDT[dtype])
+        b = g.generate(30, dtype).cpu().numpy().view(NPDT[dtype])          # bulk kernel continues
+        c = g.device_api_fill(13, dtype).cpu().numpy().view(NPDT[dtype])
+        assert g.last_kernel == "devapi_example"
+        st = g.state()
+        g.close()
+        w = Workload("devapi", gen, seed, ns, L, 64, dtype)
+        want, wst = oracle_run(w)
+        assert_same(w, np.concatenate([a, b, c], 0), want)
+        assert st == wst
+
+
 def got_dtype(dtype):
     return {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
 
