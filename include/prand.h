@@ -139,6 +139,21 @@ int prand_generate_seq_f32(prand_state *st, float *out, uint64_t length, void *c
 int prand_generate_seq_f64(prand_state *st, double *out, uint64_t length, void *cuda_stream);
 
 /*
+ * prand_generate_strided_{u32,f32,f64} -- the generator that skips ahead after every output
+ *   (PAPER.md:226 and Table 3: sequences that jump 2^n per step).  out[i * n_streams
+ *   + s] = the output of stream s at position P_s + i * stride (P_s = its current position), stride =
+ *   stride_mant * 2^stride_log2 >= 1; afterwards every stream has advanced n_per_stream * stride.
+ *   One jump per output row (the operator is prepared once): meant for testing skip-ahead sequences,
+ *   not for bulk throughput.  The library keeps a second copy of the state while it runs.
+ */
+int prand_generate_strided_u32(prand_state *st, uint32_t *out, uint64_t n_per_stream, uint64_t stride_mant,
+                               unsigned stride_log2, void *cuda_stream);
+int prand_generate_strided_f32(prand_state *st, float *out, uint64_t n_per_stream, uint64_t stride_mant,
+                               unsigned stride_log2, void *cuda_stream);
+int prand_generate_strided_f64(prand_state *st, double *out, uint64_t n_per_stream, uint64_t stride_mant,
+                               unsigned stride_log2, void *cuda_stream);
+
+/*
  * Device-callable API (the generators can be called from a user's kernel).
  * include/prand_device.cuh holds the header-only __device__ generators; these calls give a kernel
  * access to the library's device-resident state (layout documented in that header; the pointer stays

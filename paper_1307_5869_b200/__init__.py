@@ -45,6 +45,9 @@ _SIGS = {
     "prand_device_api_fill_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_device_api_fill_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_device_api_fill_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_generate_strided_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint, C.c_void_p]),
+    "prand_generate_strided_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint, C.c_void_p]),
+    "prand_generate_strided_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint, C.c_void_p]),
     "prand_free": (C.c_int, [C.c_void_p]),
     "prand_fill_u32": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p]),
     "prand_launch_count": (C.c_uint64, []),
@@ -269,6 +272,16 @@ class Generator:
         tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
         out = torch.empty((n_per_stream, self.n_streams), dtype=tdt, device="cuda")
         _generate("prand_device_api_fill_" + dtype, self._h, out.data_ptr(), n_per_stream, stream)
+        return out
+
+    def generate_strided(self, n_per_stream: int, stride: int, dtype: str = "u32", stream=None):
+        """Row i = every stream's output at its position + i * stride (the skip-per-step generator)."""
+        import torch
+        tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
+        out = torch.empty((n_per_stream, self.n_streams), dtype=tdt, device="cuda")
+        mant, log2 = split_dist(stride)
+        _check(getattr(lib(), "prand_generate_strided_" + dtype)(self._h, out.data_ptr(), n_per_stream, mant, log2,
+                                                                 _stream_ptr(stream)), "prand_generate_strided")
         return out
 
     def generate_seq(self, length: int, dtype: str = "u32", out=None, stream=None):

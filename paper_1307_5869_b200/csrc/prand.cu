@@ -397,20 +397,21 @@ extern "C" int prand_init(prand_state **out, int gen, uint64_t seed, uint64_t n_
 // ==================================================================================================
 // prand_jump (a2)
 // ==================================================================================================
-extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_log2, void *cuda_stream)
+namespace {
+// upload the operator of distance n into st->d_ops
+int jump_prepare(prand_state *st, Dist n, cudaStream_t stream)
 {
-    if (!st) return PRAND_ERR_ARG;
-    if (steps_log2 > 32768) return PRAND_ERR_ARG;
-    if (steps_mant == 0) return PRAND_OK;
-    cudaStream_t stream = (cudaStream_t)cuda_stream;
-    st->last_stream = stream;
-    Dist n = {steps_mant, steps_log2};
     std::vector<unsigned char> ops;
     int rc = build_level_ops(st->gen, n, 1, ops);
     if (rc) return rc;
     rc = ensure_ops(st, ops.size());
     if (rc) return rc;
     UPLOAD(st->d_ops, ops.data(), ops.size(), stream);
+    return PRAND_OK;
+}
+// apply the operator in st->d_ops to every stream
+int jump_launch(prand_state *st, cudaStream_t stream)
+{
     LaunchInfo li;
     if (st->gen == PRAND_MT19937) {
         uint32_t *d = (uint32_t *)st->d_state[st->cur];
@@ -427,6 +428,22 @@ extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_l
         CU(launch_jump(stream, st->gen, a, &li));
     }
     note(st, li);
+    return PRAND_OK;
+}
+}  // namespace
+
+extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_log2, void *cuda_stream)
+{
+    if (!st) return PRAND_ERR_ARG;
+    if (steps_log2 > 32768) return PRAND_ERR_ARG;
+    if (steps_mant == 0) return PRAND_OK;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    st->last_stream = stream;
+    Dist n = {steps_mant, steps_log2};
+    int rc = jump_prepare(st, n, stream);
+    if (rc) return rc;
+    rc = jump_launch(st, stream);
+    if (rc) return rc;
     if (steps_log2 >= 4 || steps_mant >= 16) st->gm_clean = true;   // past the 2-adic transient
     return PRAND_OK;
 }
@@ -691,6 +708,57 @@ int generate_seq(prand_state *st, void *out, uint64_t length, int dtype, cudaStr
 }
 
 }  // namespace
+
+// prand_generate_strided_* (SURVEY.md 8(f)4): the sequence that skips ahead after every output
+// (Table 3 PAPER.md:249-275 tests such sequences for skips of 2^n).  Row i holds every
+// stream's output at position P + i * stride: the output is produced from a copy of the state, the
+// state itself jumps by `stride` with one prepared operator.
+namespace {
+int generate_strided(prand_state *st, void *out, uint64_t n, int dtype, Dist stride, cudaStream_t stream)
+{
+    if (!st || (!out && n)) return PRAND_ERR_ARG;
+    if (stride.mant == 0 || stride.log2 > 32768) return PRAND_ERR_ARG;
+    if (n == 0) return PRAND_OK;
+    if (stride.mant == 1 && stride.log2 == 0) return generate(st, out, n, dtype, stream);
+    st->last_stream = stream;
+    const size_t esz = dtype == DT_F64 ? 8 : 4;
+    if ((uintptr_t)out % esz) return PRAND_ERR_ARG;
+    int rc = ensure_second_buffer(st);
+    if (rc) return rc;
+    rc = jump_prepare(st, stride, stream);
+    if (rc) return rc;
+    const bool clean0 = st->gm_clean;
+    for (uint64_t i = 0; i < n; i++) {
+        const int cur = st->cur;
+        CU(cudaMemcpyAsync(st->d_state[1 - cur], st->d_state[cur], st->bytes, cudaMemcpyDeviceToDevice, stream));
+        st->cur = 1 - cur;                                   // one output from the copy
+        rc = generate(st, (char *)out + i * st->ns * esz, 1, dtype, stream);
+        st->cur = cur;
+        if (rc) return rc;
+        rc = jump_launch(st, stream);
+        if (rc) return rc;
+        if (stride.log2 >= 4 || stride.mant >= 16) st->gm_clean = true;
+        else st->gm_clean = clean0 && st->gm_clean;
+    }
+    return PRAND_OK;
+}
+}  // namespace
+
+extern "C" int prand_generate_strided_u32(prand_state *st, uint32_t *out, uint64_t n, uint64_t stride_mant,
+                                          unsigned stride_log2, void *s)
+{
+    return generate_strided(st, out, n, DT_U32, Dist{stride_mant, stride_log2}, (cudaStream_t)s);
+}
+extern "C" int prand_generate_strided_f32(prand_state *st, float *out, uint64_t n, uint64_t stride_mant,
+                                          unsigned stride_log2, void *s)
+{
+    return generate_strided(st, out, n, DT_F32, Dist{stride_mant, stride_log2}, (cudaStream_t)s);
+}
+extern "C" int prand_generate_strided_f64(prand_state *st, double *out, uint64_t n, uint64_t stride_mant,
+                                          unsigned stride_log2, void *s)
+{
+    return generate_strided(st, out, n, DT_F64, Dist{stride_mant, stride_log2}, (cudaStream_t)s);
+}
 
 extern "C" int prand_generate_seq_u32(prand_state *st, uint32_t *out, uint64_t length, void *s)
 {

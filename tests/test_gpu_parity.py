@@ -277,6 +277,28 @@ def test_device_callable_api_matches_oracle_and_bulk_kernels(gen):
         assert st == wst
 
 
+@pytest.mark.parametrize("gen", ALL_GENS)
+def test_skip_per_step_generator(gen):
+    """PAPER.md:226, Table 3: the sequence that outputs one number and jumps `stride` ahead."""
+    need_gpu()
+    seed = workloads.SEED.get(gen, 1)
+    ns, L = (2, 1000) if gen == "mt19937" else (37, workloads.BLOCK_LEN[gen])
+    for stride, n in ((1, 5), (2, 6), (3 * 2**20, 4), (2**40, 3)):
+        if (gen == "gm19" and stride > 2**20) or (gen == "mt19937" and stride > 2**30):
+            continue
+        g = P.Generator(gen, seed, ns, L)
+        got = g.generate_strided(n, stride, "u32").cpu().numpy().view(np.uint32)
+        st = g.state()
+        g.close()
+        for s in range(ns):
+            o = oracle.State(gen, seed).jump(s * L)
+            for i in range(n):
+                assert got[i, s] == o.copy().fill(1, "u32")[0], f"{gen}: stride {stride} row {i} stream {s}"
+                o.jump(stride)
+            per = len(st) // ns
+            assert st[s * per:(s + 1) * per] == o.export()
+
+
 def got_dtype(dtype):
     return {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
 
