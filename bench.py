@@ -371,6 +371,11 @@ def run_sweep(args):
         w = workloads.ALL[name]
         tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[w.dtype]
         gen_fn = {"u32": P.prand_generate_u32, "f32": P.prand_generate_f32, "f64": P.prand_generate_f64}[w.dtype]
+        if w.seq:
+            seq_name = "prand_generate_seq_" + w.dtype
+
+            def gen_fn(h, ptr, n, _name=seq_name):
+                P._generate(_name, h, ptr, n, None)
         out = torch.empty((w.n_per_stream, w.n_streams), dtype=tdt, device="cuda")
         init_ms = []
         h = None

@@ -24,25 +24,31 @@ __device__ __forceinline__ uint32_t mt_recur(uint32_t xi, uint32_t xi1, uint32_t
 // ---- eq. 10 in correlation form -----------------------------------------------------------------
 // One CTA per destination stream.  The source window is extended to x_0..x_{19937+623} in shared
 // memory (227 independent words per round), then output word j is the XOR of x_{i+j}
-// over the set coefficients a_i of g_v.
+// over the set coefficients a_i of g_v.  The coefficients are expanded, 2048 at a time, into a list of
+// set positions in shared memory, so that the accumulation loop has no bit scan and runs eight
+// positions (24 independent shared loads per thread) at a time; the list is padded with a position
+// whose words are zero.
 constexpr int APPLY_THREADS = 256;
-constexpr int APPLY_XWORDS = DEG + NW;
-constexpr size_t APPLY_SMEM = (size_t)(APPLY_XWORDS + NW) * sizeof(uint32_t);
+constexpr int APPLY_XWORDS = DEG + NW;                      // 20561
+constexpr int APPLY_ZERO = APPLY_XWORDS;                    // x[APPLY_ZERO .. +APPLY_ZPAD) = 0
+constexpr int APPLY_ZPAD = 771;                             // >= 768, makes the list 16-byte aligned
+constexpr int APPLY_CHUNK = 64;                             // polynomial words per expansion
+constexpr int APPLY_LIST = APPLY_CHUNK * 32 + 8;            // positions (u16) incl. padding
+constexpr size_t APPLY_SMEM = (size_t)(APPLY_XWORDS + APPLY_ZPAD) * sizeof(uint32_t) + APPLY_LIST * sizeof(uint16_t) + 16;
 
 __global__ void __launch_bounds__(APPLY_THREADS)
 mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
                      uint64_t src_back, const MtOp *__restrict__ op)
 {
-    extern __shared__ uint32_t smem[];
-    uint32_t *x = smem;                    // APPLY_XWORDS
-    uint32_t *poly = smem + APPLY_XWORDS;  // NW
+    extern __shared__ __align__(16) uint32_t smem[];
+    uint32_t *x = smem;                                                      // APPLY_XWORDS + APPLY_ZPAD
+    uint16_t *list = reinterpret_cast<uint16_t *>(smem + APPLY_XWORDS + APPLY_ZPAD);  // APPLY_LIST
+    int *meta = reinterpret_cast<int *>(list + APPLY_LIST);                  // [0] warp-0 total, [1] count
     const int tid = threadIdx.x;
     const uint64_t dst = dst0 + blockIdx.x;
     const uint32_t *src = st_src + (dst - src_back) * NW;
-    for (int j = tid; j < NW; j += APPLY_THREADS) {
-        x[j] = src[j];
-        poly[j] = op->w[j];
-    }
+    for (int j = tid; j < NW; j += APPLY_THREADS) x[j] = src[j];
+    for (int j = tid; j < APPLY_ZPAD; j += APPLY_THREADS) x[APPLY_ZERO + j] = 0;
     __syncthreads();
     for (int r0 = 0; r0 < DEG; r0 += 227) {
         int k = r0 + tid;
@@ -53,15 +59,44 @@ mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
     uint32_t acc0 = 0, acc1 = 0, acc2 = 0;
     const uint32_t *x0 = x + tid, *x1 = x + tid + 256;
     const uint32_t *x2 = x + (tid + 512 < NW ? tid + 512 : 0);
-    for (int wi = 0; wi < NW; wi++) {
-        uint32_t pw = poly[wi];            // uniform over the CTA
-        while (pw) {
-            int i = wi * 32 + (__ffs(pw) - 1);
-            pw &= pw - 1;
-            acc0 ^= x0[i];
-            acc1 ^= x1[i];
-            acc2 ^= x2[i];
+    for (int c0 = 0; c0 < NW; c0 += APPLY_CHUNK) {
+        // expand polynomial words c0 .. c0+63 (threads 0..63, two warps) into the list of set positions
+        if (tid < APPLY_CHUNK) {
+            const int wi = c0 + tid;
+            uint32_t pw = wi < NW ? __ldg(&op->w[wi]) : 0u;
+            const int cnt = __popc(pw);
+            int incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+                if ((tid & 31) >= d) incl += v;
+            }
+            if (tid == 31) meta[0] = incl;
+            __syncwarp();
+            asm volatile("bar.sync 1, 64;" ::: "memory");
+            int pos = incl - cnt + (tid >= 32 ? meta[0] : 0);
+            if (tid == APPLY_CHUNK - 1) meta[1] = pos + cnt;
+            while (pw) {
+                list[pos++] = (uint16_t)(wi * 32 + (__ffs(pw) - 1));
+                pw &= pw - 1;
+            }
         }
+        __syncthreads();
+        const int n = meta[1];
+        if (tid < 8) list[n + tid] = (uint16_t)APPLY_ZERO;
+        __syncthreads();
+        for (int k = 0; k < n; k += 8) {
+            const uint4 q = *reinterpret_cast<const uint4 *>(list + k);      // eight positions, uniform
+            const uint32_t ii[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+            for (int h = 0; h < 4; h++) {
+                const int ia = ii[h] & 0xFFFF, ib = ii[h] >> 16;
+                acc0 ^= x0[ia] ^ x0[ib];
+                acc1 ^= x1[ia] ^ x1[ib];
+                acc2 ^= x2[ia] ^ x2[ib];
+            }
+        }
+        __syncthreads();
     }
     uint32_t *d = st_dst + dst * NW;
     d[tid] = tid == 0 ? (acc0 & 0x80000000u) : acc0;   // only the top bit of word 0 is state (T2)

@@ -19,6 +19,7 @@ class Workload:
     block_len: int
     n_per_stream: int
     dtype: str          # "u32" | "f32" | "f64"
+    seq: bool = False   # True: PRAND's single-sequence fill (prand_generate_seq_*), out[0..n_per_stream)
 
     @property
     def numbers(self) -> int:
@@ -50,5 +51,10 @@ C4 = [Workload("C4-gm61", "gm61", 1, 131072, 2 ** 33, 8192, "f32"),
 C5_GENS = ["gm19", "gm29", "gm55", "gq58.1", "gq58.3", "gq58.4", "lfsr113", "mrg32k3a", "mt19937"]
 C5 = [Workload(f"C5-{g}", g, SEED.get(g, 1), 2 ** 20, BLOCK_LEN[g], 2048, "u32") for g in C5_GENS]
 
-ALL = {w.name: w for w in [C1, C2, C3] + C4 + C5}
+# The paper's Table 7 task: fill an array of 2^29 doubles in GPU memory with ONE
+# sequence (the paper repeats it 100 times); the array layout is PRAND's contiguous sections.
+T7 = [Workload("T7-mrg32k3a", "mrg32k3a", 12345, 1, 0, 2 ** 29, "f64", True),
+      Workload("T7-mt19937", "mt19937", 5489, 1, 0, 2 ** 29, "f64", True)]
+
+ALL = {w.name: w for w in [C1, C2, C3] + C4 + C5 + T7}
 HEADLINE = C2        # BASELINE.json configs[1]: the configuration the bench line is quoted on
