@@ -44,6 +44,12 @@ int prand_host_mt19937_mulmod(const uint32_t *a624, const uint32_t *b624, uint32
 int prand_host_plan(int gen, uint64_t n_streams, uint64_t n_per_stream, int dtype, int sm_count,
                     uint64_t *chunk_len, uint64_t *n_chunks);
 
+/*
+ * Section plan of prand_generate_seq_* (Table 5): `length` outputs of one sequence are
+ * cut into n_sections sections of sec_len (a multiple of 32; the last one may be shorter).
+ */
+int prand_host_plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec_len);
+
 #ifdef __cplusplus
 }
 #endif

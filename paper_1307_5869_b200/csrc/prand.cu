@@ -648,7 +648,7 @@ void plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec
 {
     // enough sections to fill the GPU, sections long enough to amortise the jump to their start
     const uint64_t min_len = gen == PRAND_MT19937 ? 8 * 624 : 1024;
-    const uint64_t max_sec = gen == PRAND_MT19937 ? 4096 : 65536;
+    const uint64_t max_sec = gen == PRAND_MT19937 ? 1024 : 65536;   // MT19937: one 0.2 ms jump level per doubling
     uint64_t S = length / min_len;
     if (S > max_sec) S = max_sec;
     if (S < 1) S = 1;
@@ -983,6 +983,14 @@ extern "C" int prand_host_mt19937_mulmod(const uint32_t *a624, const uint32_t *b
     std::memcpy(b.w, b624, sizeof b.w);
     host::mt19937_mulmod(r, a, b);
     std::memcpy(r624, r.w, sizeof r.w);
+    return PRAND_OK;
+}
+
+extern "C" int prand_host_plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec_len)
+{
+    if (gen < 0 || gen >= PRAND_NGEN) return PRAND_ERR_GEN;
+    if (!n_sections || !sec_len || length == 0) return PRAND_ERR_ARG;
+    plan_sections(gen, length, n_sections, sec_len);
     return PRAND_OK;
 }
 

@@ -164,3 +164,17 @@ def test_plan_covers_all_rows(gen):
     assert P.prand_host_plan("lfsr113", 2**20, 2048, "u32", 148) == (2048, 1)
     # config 1 (1024 streams x 4096) must be cut to fill the GPU
     assert P.prand_host_plan("lfsr113", 1024, 4096, "u32", 148)[1] > 1
+
+
+def test_section_plan_covers_the_array_exactly_once():
+    """prand_generate_seq_* (PAPER.md:382): sections tile [0, length) with no gap, no empty section."""
+    import ctypes as C
+    for gen in ("lfsr113", "mrg32k3a", "mt19937", "gm61"):
+        for length in (1, 31, 1024, 4999, 8 * 624 * 2, 10**6 + 7, 2**29, 2**33 + 5):
+            S, L = C.c_uint64(), C.c_uint64()
+            assert P.lib().prand_host_plan_sections(P.gen_id(gen), length, C.byref(S), C.byref(L)) == 0
+            S, L = S.value, L.value
+            assert S >= 1 and L >= 1 and L % 32 == 0
+            assert (S - 1) * L < length <= S * L
+            assert S <= (1024 if gen == "mt19937" else 65536)
+    assert P.lib().prand_host_plan_sections(0, 0, C.byref(C.c_uint64()), C.byref(C.c_uint64())) == -2
