@@ -147,6 +147,10 @@ template <> struct Gm<PRAND_GM61> {
 
 // GM55: register word Y = 2^13 y (the 51-bit residue mod p in the top bits), arithmetic mod
 // M = 2^13 p = 2^64 - C, C = 129 * 2^13, exactly as for GM61.
+// The multipliers are read from constant memory so that the compiler keeps 256 * YN as a 32x32+64
+// multiply-add on the FMA pipe instead of a chain of 64-bit shifts and masks on the ALU pipe.
+static __constant__ uint32_t gm55_kq[2] = {256u, 176u};
+
 template <> struct Gm<PRAND_GM55> {
     typedef uint64_t W;
     typedef uint64_t R;
@@ -158,12 +162,13 @@ template <> struct Gm<PRAND_GM55> {
     __device__ static __forceinline__ W store(R Y) { return (Y >> 13) << 4; }
     __device__ static __forceinline__ R step(R YP, R YN)
     {
+        const uint32_t K = gm55_kq[0], Q = gm55_kq[1];
         const uint64_t D = M - YP;
         const uint32_t dl = (uint32_t)D, dh = (uint32_t)(D >> 32);
         const uint32_t nl = (uint32_t)YN, nh = (uint32_t)(YN >> 32);
-        uint64_t c0 = (uint64_t)nl * 256u + (uint64_t)dl * 176u;                     // < 432 * 2^32
-        uint64_t c1 = (uint64_t)nh * 256u + (c0 >> 32);
-        c1 = (uint64_t)dh * 176u + c1;                                               // top limb A < 432
+        uint64_t c0 = (uint64_t)nl * K + (uint64_t)dl * Q;                           // < 432 * 2^32
+        uint64_t c1 = (uint64_t)nh * K + (c0 >> 32);
+        c1 = (uint64_t)dh * Q + c1;                                                  // top limb A < 432
         const uint32_t ac = (uint32_t)(c1 >> 32) * C + C;                            // (A + 1) C < 2^29
         uint32_t sl, sh, cy;
         asm("add.cc.u32 %0, %3, %4;\n\t"
@@ -174,20 +179,13 @@ template <> struct Gm<PRAND_GM55> {
         if (cy == 0) Sx -= C;
         return Sx;
     }
-    // floor(16 y / p) = floor(16 Y / M): with h = Y >> 60 and L = 16 Y mod 2^64, 16 Y = h M + h C + L,
-    // so the digit is h plus the carry out of L + (h + 1) C
+    // floor(16 y / p) = floor(16 Y / M): with h = Y >> 60, 16 Y = h 2^64 + L = h M + (h C + L), so the
+    // digit is h + [L + (h + 1) C >= 2^64] = floor((16 Y + (h + 1) C) / 2^64) = (Y + (h + 1) C / 16) >> 60
     __device__ static __forceinline__ void pack(uint32_t &word, R Y, const int J)
     {
-        const uint32_t yl = (uint32_t)Y, yh = (uint32_t)(Y >> 32);
-        const uint32_t h = yh >> 28;
-        const uint32_t ll = yl << 4, lh = __funnelshift_l(yl, yh, 4);
-        const uint32_t hc = h * C + C;
-        uint32_t t0, t1, d;
-        asm("add.cc.u32 %0, %3, %4;\n\t"
-            "addc.cc.u32 %1, %5, 0;\n\t"
-            "addc.u32 %2, %6, 0;"
-            : "=r"(t0), "=r"(t1), "=r"(d) : "r"(ll), "r"(hc), "r"(lh), "r"(h));
-        word += d << (4 * J);
+        const uint32_t h = (uint32_t)(Y >> 60);
+        const uint64_t t = Y + (uint64_t)(h * (C / 16) + (C / 16));
+        word = pack_mad(word, (uint32_t)(t >> 60), 4 * J);
     }
 };
 
