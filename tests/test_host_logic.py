@@ -178,3 +178,24 @@ def test_section_plan_covers_the_array_exactly_once():
             assert (S - 1) * L < length <= S * L
             assert S <= (1024 if gen == "mt19937" else 65536)
     assert P.lib().prand_host_plan_sections(0, 0, C.byref(C.c_uint64()), C.byref(C.c_uint64())) == -2
+
+
+def test_bench_reference_arm_prints_the_contract_line():
+    """bench.py --impl reference (this tier's reference arm = the oracle on the host cores) prints one
+    JSON line with the contract's keys; no GPU is touched."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "0"], capture_output=True, text=True, timeout=300, cwd=root)
+    assert out.returncode == 0, out.stderr
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for key in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better",
+                "scaling", "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert key in d, key
+    assert d["impl"] == "reference" and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and "workload" in d["config"]
