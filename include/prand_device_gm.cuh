@@ -34,7 +34,7 @@ template <> struct Gm<PRAND_GM19> {
     typedef uint32_t W;
     typedef uint32_t R;
     static constexpr int S = 32;
-    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false;
+    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint32_t G = (1u << 19) - 1;
     __device__ static __forceinline__ R load(W x) { return x; }
     __device__ static __forceinline__ W store(R x) { return x; }
@@ -52,7 +52,7 @@ template <> struct Gm<PRAND_GM29> {
     typedef uint32_t W;
     typedef uint32_t R;
     static constexpr int S = 32;
-    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false;
+    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint32_t G = (1u << 29) - 3;
     __device__ static __forceinline__ R load(W x) { return x; }
     __device__ static __forceinline__ W store(R x) { return x; }
@@ -74,7 +74,7 @@ template <> struct Gm<PRAND_GM31> {
     typedef uint32_t W;
     typedef uint32_t R;
     static constexpr int S = 32;
-    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false;
+    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint32_t G = (1u << 31) - 1;
     __device__ static __forceinline__ R load(W x) { return x; }
     __device__ static __forceinline__ W store(R x) { return x; }
@@ -97,11 +97,13 @@ template <> struct Gm<PRAND_GM31> {
 // bits exactly when X' >= M, and then S mod 2^64 = X' - M; otherwise X' = S - 8.  M - XP = ~XP with the
 // three low bits cleared (two LOP3); the digit (bit 60 of x) is bit 63 of X, shifted into the output
 // word by one funnel shift.
+static __constant__ uint32_t gm61_eight[1] = {8u};        // from constant memory: keeps 8 A an IMAD (FMA pipe)
+
 template <> struct Gm<PRAND_GM61> {
     typedef uint64_t W;
     typedef uint64_t R;
     static constexpr int S = 32;
-    static constexpr bool PACK_DESCENDING = true, NEEDS_CLEAN = false;
+    static constexpr bool PACK_DESCENDING = true, NEEDS_CLEAN = false, HAS_FAST = true;
     __device__ static __forceinline__ R load(W x) { return x << 3; }
     __device__ static __forceinline__ W store(R x) { return x >> 3; }
     __device__ static __forceinline__ R step(R XP, R XN)
@@ -131,6 +133,37 @@ template <> struct Gm<PRAND_GM61> {
             : "=l"(S) : "l"(XP), "l"(XN));
         return S;
     }
+    // Optimistic form of the same step for the bulk kernels: X' = lo64 + 8 A without the test against
+    // M.  If the middle limb c1l of T is at most 2^32 - 3, the sum neither carries out of 64 bits nor
+    // reaches M, so the result is already canonical; otherwise (probability 2^-31 per point) the
+    // caller must discard it and call step().  `watch` collects the maximum of c1l over a group of points.
+    __device__ static __forceinline__ R step_fast(R XP, R XN, uint32_t &watch)
+    {
+        uint64_t S;
+        uint32_t mid;
+        asm("{\n\t.reg .u32 pl, ph, nl, nh, yl, yh, c0l, c0h, c1l, c1h, a8, sl, sh;\n\t"
+            ".reg .u64 c0, c1;\n\t"
+            "mov.b64 {pl, ph}, %2;\n\t"
+            "mov.b64 {nl, nh}, %3;\n\t"
+            "xor.b32 yl, pl, 0xFFFFFFF8;\n\t"
+            "not.b32 yh, ph;\n\t"
+            "mul.wide.u32 c0, nl, 24;\n\t"
+            "mad.wide.u32 c0, yl, 74, c0;\n\t"
+            "mov.b64 {c0l, c0h}, c0;\n\t"
+            "mov.b64 c1, {c0h, 0};\n\t"
+            "mad.wide.u32 c1, nh, 24, c1;\n\t"
+            "mad.wide.u32 c1, yh, 74, c1;\n\t"
+            "mov.b64 {c1l, c1h}, c1;\n\t"
+            "mul.lo.u32 a8, c1h, %4;\n\t"
+            "add.cc.u32 sl, c0l, a8;\n\t"
+            "addc.u32 sh, c1l, 0;\n\t"
+            "mov.b64 %0, {sl, sh};\n\t"
+            "mov.u32 %1, c1l;\n\t}"
+            : "=l"(S), "=r"(mid) : "l"(XP), "l"(XN), "r"(gm61_eight[0]));
+        watch = max(watch, mid);
+        return S;
+    }
+    static constexpr uint32_t WATCH_LIMIT = 0xFFFFFFFEu;      // watch >= limit: redo the group with step()
     __device__ static __forceinline__ void pack(uint32_t &word, R X, const int J)
     {
         word = __funnelshift_l((uint32_t)(X >> 32), word, 1);     // (word << 1) | bit 63 of X
@@ -149,13 +182,14 @@ template <> struct Gm<PRAND_GM61> {
 // M = 2^13 p = 2^64 - C, C = 129 * 2^13, exactly as for GM61.
 // The multipliers are read from constant memory so that the compiler keeps 256 * YN as a 32x32+64
 // multiply-add on the FMA pipe instead of a chain of 64-bit shifts and masks on the ALU pipe.
-static __constant__ uint32_t gm55_kq[2] = {256u, 176u};
+static __constant__ uint32_t gm55_kq[3] = {256u, 176u, 129u << 13};
 
 template <> struct Gm<PRAND_GM55> {
     typedef uint64_t W;
     typedef uint64_t R;
     static constexpr int S = 8;
-    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = true;
+    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = true, HAS_FAST = true;
+    static constexpr uint32_t WATCH_LIMIT = 0xFFFFFFFEu;
     static constexpr uint32_t C = 129u << 13;
     static constexpr uint64_t M = 0ull - C;
     __device__ static __forceinline__ R load(W x) { return x << 9; }               // x = 16 y
@@ -179,6 +213,21 @@ template <> struct Gm<PRAND_GM55> {
         if (cy == 0) Sx -= C;
         return Sx;
     }
+    // Optimistic form (see GM61): Y' = lo64 + A C is canonical whenever the middle limb of T is at most
+    // 2^32 - 3; `watch` collects the maximum of that limb, the caller falls back to step() otherwise.
+    __device__ static __forceinline__ R step_fast(R YP, R YN, uint32_t &watch)
+    {
+        const uint32_t K = gm55_kq[0], Q = gm55_kq[1];
+        const uint64_t D = M - YP;
+        const uint32_t dl = (uint32_t)D, dh = (uint32_t)(D >> 32);
+        const uint32_t nl = (uint32_t)YN, nh = (uint32_t)(YN >> 32);
+        uint64_t c0 = (uint64_t)nl * K + (uint64_t)dl * Q;
+        uint64_t c1 = (uint64_t)nh * K + (c0 >> 32);
+        c1 = (uint64_t)dh * Q + c1;
+        watch = max(watch, (uint32_t)c1);
+        const uint64_t lo64 = (c1 << 32) | (uint32_t)c0;
+        return lo64 + (uint64_t)((uint32_t)(c1 >> 32) * gm55_kq[2]);
+    }
     // floor(16 y / p) = floor(16 Y / M): with h = Y >> 60, 16 Y = h 2^64 + L = h M + (h C + L), so the
     // digit is h + [L + (h + 1) C >= 2^64] = floor((16 Y + (h + 1) C) / 2^64) = (Y + (h + 1) C / 16) >> 60
     __device__ static __forceinline__ void pack(uint32_t &word, R Y, const int J)
@@ -193,7 +242,7 @@ template <int VB, int SS> struct Gq58 {
     typedef uint64_t W;
     typedef uint32_t R;
     static constexpr int S = SS;
-    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = true;
+    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = true, HAS_FAST = false;
     static constexpr uint32_t P = (1u << 29) - 3;
     __device__ static __forceinline__ R load(W x) { return (uint32_t)(x >> 29); }  // x = 2^29 y
     __device__ static __forceinline__ W store(R y) { return (uint64_t)y << 29; }
@@ -237,7 +286,7 @@ template <> struct GmPlain<PRAND_GM55> {
     typedef uint64_t W;
     typedef uint64_t R;
     static constexpr int S = 8;
-    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false;
+    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint64_t P = (1ull << 51) - 129;
     static constexpr uint64_t G = 16ull * P;
     __device__ static __forceinline__ R load(W x) { return x; }
@@ -262,7 +311,7 @@ template <int VB, int SS> struct Gq58Plain {
     typedef uint64_t W;
     typedef uint64_t R;
     static constexpr int S = SS;
-    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false;
+    static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint64_t P = (1ull << 29) - 3;
     static constexpr uint64_t G = P << 29;
     __device__ static __forceinline__ R load(W x) { return x; }

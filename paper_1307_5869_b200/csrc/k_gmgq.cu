@@ -83,7 +83,7 @@ template <class Tr, int LP, int DT, int MINB>
 __global__ void __launch_bounds__(128, MINB)
 gm_gen_kernel(const typename Tr::W *st_in, typename Tr::W *st_out,
               typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n, uint64_t chunk_len,
-              uint64_t n_chunks, const GmOp *__restrict__ chunk_ops, Barrett B)
+              uint64_t n_chunks, const GmOp *__restrict__ chunk_ops, Barrett B, uint32_t watch_limit)
 {
     typedef typename Tr::W W;
     typedef typename Tr::R R;
@@ -119,11 +119,40 @@ gm_gen_kernel(const typename Tr::W *st_in, typename Tr::W *st_out,
     auto step_word = [&](auto par) -> uint32_t {
         constexpr bool PAR = decltype(par)::value;
         uint32_t word = 0;
+        if constexpr (Tr::HAS_FAST) {
+            // optimistic steps in groups of (up to) 8 points; a group whose watch value reaches the
+            // limit (probability ~2^-28) is recomputed with the exact step before it is committed
+            constexpr int GRP = PPL < 8 ? PPL : 8;
 #pragma unroll
-        for (int jj = 0; jj < PPL; jj++) {
-            const int j = Tr::PACK_DESCENDING ? PPL - 1 - jj : jj;
-            if (!PAR) { xP[j] = Tr::step(xP[j], xN[j]); Tr::pack(word, xP[j], j); }
-            else { xN[j] = Tr::step(xN[j], xP[j]); Tr::pack(word, xN[j], j); }
+            for (int g0 = 0; g0 < PPL; g0 += GRP) {
+                R nw[GRP];
+                uint32_t watch = 0;
+#pragma unroll
+                for (int jj = 0; jj < GRP; jj++) {
+                    const int j = Tr::PACK_DESCENDING ? PPL - 1 - (g0 + jj) : g0 + jj;
+                    nw[jj] = PAR ? Tr::step_fast(xN[j], xP[j], watch) : Tr::step_fast(xP[j], xN[j], watch);
+                }
+                if (watch >= watch_limit) {
+#pragma unroll
+                    for (int jj = 0; jj < GRP; jj++) {
+                        const int j = Tr::PACK_DESCENDING ? PPL - 1 - (g0 + jj) : g0 + jj;
+                        nw[jj] = PAR ? Tr::step(xN[j], xP[j]) : Tr::step(xP[j], xN[j]);
+                    }
+                }
+#pragma unroll
+                for (int jj = 0; jj < GRP; jj++) {
+                    const int j = Tr::PACK_DESCENDING ? PPL - 1 - (g0 + jj) : g0 + jj;
+                    if (!PAR) xP[j] = nw[jj]; else xN[j] = nw[jj];
+                    Tr::pack(word, nw[jj], j);
+                }
+            }
+        } else {
+#pragma unroll
+            for (int jj = 0; jj < PPL; jj++) {
+                const int j = Tr::PACK_DESCENDING ? PPL - 1 - jj : jj;
+                if (!PAR) { xP[j] = Tr::step(xP[j], xN[j]); Tr::pack(word, xP[j], j); }
+                else { xN[j] = Tr::step(xN[j], xP[j]); Tr::pack(word, xN[j], j); }
+            }
         }
         return word;
     };
@@ -181,6 +210,18 @@ gm_gen_kernel(const typename Tr::W *st_in, typename Tr::W *st_out,
     }
 }
 
+// Limit of the optimistic steps' watch value (Tr::WATCH_LIMIT); the test hook PRAND_GM_WATCH lowers it
+// so that the exact fallback runs often (0: always).
+template <class Tr> uint32_t gm_watch_limit()
+{
+    if constexpr (Tr::HAS_FAST) {
+        if (const char *env = std::getenv("PRAND_GM_WATCH")) return (uint32_t)std::strtoul(env, nullptr, 0);
+        return Tr::WATCH_LIMIT;
+    } else {
+        return 0xFFFFFFFFu;
+    }
+}
+
 template <class Tr, int LP, int DT, int MINB>
 cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a, const Barrett &B)
 {
@@ -190,7 +231,7 @@ cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a, const Barrett &B)
     unsigned blocks = (unsigned)ceil_div_u64(lanes, 128);
     gm_gen_kernel<Tr, LP, DT, MINB><<<blocks, 128, 0, stream>>>((const W *)a.st_in, (W *)a.st_out, (T *)a.out,
                                                                 a.n_streams, a.n, a.chunk_len, a.n_chunks,
-                                                                (const GmOp *)a.chunk_ops, B);
+                                                                (const GmOp *)a.chunk_ops, B, gm_watch_limit<Tr>());
     return cudaGetLastError();
 }
 
@@ -241,9 +282,9 @@ cudaError_t gm_generate(cudaStream_t stream, int gen, const GenArgs &a, LaunchIn
     case PRAND_GM29: li->kernel = "gm29_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM29>, 1>(stream, a, B);
     case PRAND_GM31: li->kernel = "gm31_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM31>, 1>(stream, a, B);
     case PRAND_GM61:
+        if (lp == 1) { li->kernel = "gm61_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM61>, 1, 2>(stream, a, B); }
         if (lp == 2) { li->kernel = "gm61_gen<LP=2>"; return dispatch_dt<Gm<PRAND_GM61>, 2>(stream, a, B); }
-        if (lp == 4) { li->kernel = "gm61_gen<LP=4>"; return dispatch_dt<Gm<PRAND_GM61>, 4>(stream, a, B); }
-        li->kernel = "gm61_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM61>, 1, 2>(stream, a, B);
+        li->kernel = "gm61_gen<LP=4>"; return dispatch_dt<Gm<PRAND_GM61>, 4>(stream, a, B);
     case PRAND_GM55:
         if (!a.clean) { li->kernel = "gm55_gen<plain>"; return dispatch_dt<GmPlain<PRAND_GM55>, 1>(stream, a, B); }
         li->kernel = "gm55_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM55>, 1>(stream, a, B);

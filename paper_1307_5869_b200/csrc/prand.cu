@@ -472,7 +472,10 @@ void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t 
         uint64_t per_thread_streams = 1, lanes_per_stream = 1, min_len = 64;
         if (gen == PRAND_LFSR113) per_thread_streams = 4;
         else if (gen == PRAND_MRG32K3A) per_thread_streams = dtype == DT_F64 ? 2 : 4;
-        else min_len = 128;
+        else {
+            min_len = 128;
+            if (gen == PRAND_GM61) lanes_per_stream = 4;
+        }
         uint64_t threads = ns * lanes_per_stream / per_thread_streams;
         if (threads == 0) threads = 1;
         // one balanced wave: as many equal chunks as fit the threads resident at once, never more

@@ -299,6 +299,25 @@ def test_skip_per_step_generator(gen):
             assert st[s * per:(s + 1) * per] == o.export()
 
 
+@pytest.mark.parametrize("gen", ["gm61", "gm55"])
+@pytest.mark.parametrize("limit", ["0", "0xC0000000"])
+def test_optimistic_steps_fall_back_exactly(gen, limit, monkeypatch):
+    """GM61 / GM55 run an optimistic modular step and redo a group of points with the exact step when
+    the watched limb reaches a limit (probability ~2^-28 in production).  Lowering the limit makes the
+    fallback run always ("0") or for a quarter of the points: the numbers must not change."""
+    need_gpu()
+    monkeypatch.setenv("PRAND_GM_WATCH", limit)
+    for lp in ("1", "4") if gen == "gm61" else ("1",):
+        monkeypatch.setenv("PRAND_GM_LP", lp)
+        w = Workload("watch", gen, 1, 70, workloads.BLOCK_LEN[gen], 37, "u32")
+        got, st, _ = lib_run(w, calls=[20, 17])
+        want, wst = oracle_run(w)
+        assert_same(w, got, want)
+        assert st == wst
+    monkeypatch.delenv("PRAND_GM_WATCH")
+    monkeypatch.delenv("PRAND_GM_LP")
+
+
 def got_dtype(dtype):
     return {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
 
