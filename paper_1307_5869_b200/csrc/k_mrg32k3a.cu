@@ -7,6 +7,7 @@
 // Reduction uses 2^32 = 209 (mod m1) and 2^32 = 22853 (mod m2): fold the high word down twice.
 // State layout (SoA): word w of stream s at st[w * n_streams + s], w = x_n, x_{n-1}, x_{n-2},
 // y_n, y_{n-1}, y_{n-2}.
+#include <cstdlib>
 #include "k_common.cuh"
 
 namespace prand {
@@ -205,14 +206,122 @@ mrg32k3a_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
     }
 }
 
+// ---- second component on the FP64 pipe (u32 / f32 output) --------------------------------------------
+// With 4-byte outputs the integer pipes, not HBM, bound the kernel above (ALU 66 %, FMA 42 %).  The
+// B200 has a third arithmetic pipe, FP64 (64 lanes/clk/SM), so the y component runs there, exactly:
+// y is kept as a double holding a *signed* representative r in [-m2/2, m2/2] (|r| < 2^31);
+//   p = 527612 r_n - 1370589 r_{n-2}            |p| <= 1898201 * m2 / 2 < 2^52: every product and the
+//                                               fused sum are integers below 2^53, i.e. exact;
+//   k = rint(p / m2) as fma(p, 1/m2, 1.5 * 2^52) - 1.5 * 2^52   (any integer within 1 of p/m2 will do);
+//   r' = fma(-k, m2, p) = p - k m2               exact, |r'| <= m2/2 (+ a few units).
+// Five FP64 instructions and no compare; the canonical residue for the output is r' + (r' < 0 ? m2 : 0)
+// after one exact double -> int32 conversion (XU pipe).
+struct MrgY { double y0, y1, y2; };
+__device__ __forceinline__ double mrg_y_in(uint32_t y) { return y >= 0x80000000u ? (double)y - 4294944443.0 : (double)y; }
+__device__ __forceinline__ uint32_t mrg_y_out(double r)
+{
+    const int32_t v = __double2int_rn(r);                 // exact: r is an integer, |r| < 2^31
+    return (uint32_t)v + (v < 0 ? M2 : 0u);
+}
+__device__ __forceinline__ double mrg_next_yd(double y0, double y2)
+{
+    const double t = __dmul_rn(-1370589.0, y2);
+    const double p = __fma_rn(527612.0, y0, t);
+    const double km = __fma_rn(p, 2.3283188252407387e-10, 6755399441055744.0);    // 1 / m2, 1.5 * 2^52
+    const double k = __dadd_rn(km, -6755399441055744.0);
+    return __fma_rn(-k, 4294944443.0, p);
+}
+
+template <int V, int DT>
+__global__ void __launch_bounds__(GEN_THREADS)
+mrg32k3a_gen_fp64y_kernel(const uint32_t *st_in, uint32_t *st_out,
+                          typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n,
+                          uint64_t chunk_len, const MrgOp *__restrict__ chunk_ops)
+{
+    typedef typename OutElem<DT>::type T;
+    const uint64_t sg = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t s0 = sg * V;
+    if (s0 >= ns) return;
+    const uint32_t c = blockIdx.y;
+
+    Mrg g[V];
+    MrgY h[V];
+#pragma unroll
+    for (int v = 0; v < V; v++) {
+        g[v] = mrg_load(st_in, ns, s0 + v);
+        if (c != 0) mrg_apply_op(chunk_ops + (c - 1), g[v]);
+        h[v].y0 = mrg_y_in(g[v].y0); h[v].y1 = mrg_y_in(g[v].y1); h[v].y2 = mrg_y_in(g[v].y2);
+    }
+    const uint64_t row0 = (uint64_t)c * chunk_len;
+    const uint64_t rows = (row0 + chunk_len < n) ? chunk_len : n - row0;
+    T *p = out + row0 * ns + s0;
+    T r[V];
+    uint32_t c1 = C1;
+    asm volatile("" : "+r"(c1));
+    uint64_t i = 0;
+#pragma unroll 1
+    for (; i + 3 <= rows; i += 3) {
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            g[v].x2 = mrg_next_x(g[v].x1, g[v].x2, c1);
+            h[v].y2 = mrg_next_yd(h[v].y0, h[v].y2);
+            r[v] = mrg_output<DT>(g[v].x2, mrg_y_out(h[v].y2));
+        }
+        store_vec<V>(p, r);
+        p += ns;
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            g[v].x1 = mrg_next_x(g[v].x0, g[v].x1, c1);
+            h[v].y1 = mrg_next_yd(h[v].y2, h[v].y1);
+            r[v] = mrg_output<DT>(g[v].x1, mrg_y_out(h[v].y1));
+        }
+        store_vec<V>(p, r);
+        p += ns;
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            g[v].x0 = mrg_next_x(g[v].x2, g[v].x0, c1);
+            h[v].y0 = mrg_next_yd(h[v].y1, h[v].y0);
+            r[v] = mrg_output<DT>(g[v].x0, mrg_y_out(h[v].y0));
+        }
+        store_vec<V>(p, r);
+        p += ns;
+    }
+#pragma unroll 1
+    for (; i < rows; i++) {                              // ragged tail: rotate by moving
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            const uint32_t nx = mrg_next_x(g[v].x1, g[v].x2, c1);
+            const double ny = mrg_next_yd(h[v].y0, h[v].y2);
+            g[v].x2 = g[v].x1; g[v].x1 = g[v].x0; g[v].x0 = nx;
+            h[v].y2 = h[v].y1; h[v].y1 = h[v].y0; h[v].y0 = ny;
+            r[v] = mrg_output<DT>(nx, mrg_y_out(ny));
+        }
+        store_vec<V>(p, r);
+        p += ns;
+    }
+    if (c == gridDim.y - 1) {
+#pragma unroll
+        for (int v = 0; v < V; v++) {
+            g[v].y0 = mrg_y_out(h[v].y0); g[v].y1 = mrg_y_out(h[v].y1); g[v].y2 = mrg_y_out(h[v].y2);
+            mrg_store(st_out, ns, s0 + v, g[v]);
+        }
+    }
+}
+
 template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
 {
     typedef typename OutElem<DT>::type T;
     const uint64_t groups = a.n_streams / V;
     dim3 grid((unsigned)ceil_div_u64(groups, GEN_THREADS), (unsigned)a.n_chunks);
-    mrg32k3a_gen_kernel<V, DT><<<grid, GEN_THREADS, 0, stream>>>(
-        (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
-        (const MrgOp *)a.chunk_ops);
+    const bool int_only = std::getenv("PRAND_MRG_INT") != nullptr;     // test hook: integer y component
+    if (DT != DT_F64 && !int_only)
+        mrg32k3a_gen_fp64y_kernel<V, DT><<<grid, GEN_THREADS, 0, stream>>>(
+            (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
+            (const MrgOp *)a.chunk_ops);
+    else
+        mrg32k3a_gen_kernel<V, DT><<<grid, GEN_THREADS, 0, stream>>>(
+            (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
+            (const MrgOp *)a.chunk_ops);
     return cudaGetLastError();
 }
 

@@ -318,6 +318,23 @@ def test_optimistic_steps_fall_back_exactly(gen, limit, monkeypatch):
     monkeypatch.delenv("PRAND_GM_LP")
 
 
+@pytest.mark.parametrize("dtype", ["u32", "f32"])
+def test_mrg32k3a_integer_and_fp64_pipe_kernels_agree_with_the_oracle(dtype, monkeypatch):
+    """With 4-byte outputs MRG32K3A's second component runs on the FP64 pipe (exact: every product and
+    fused sum is an integer below 2^53); PRAND_MRG_INT selects the all-integer kernel.  Both must be
+    the oracle's numbers, also from states whose words exceed 2^31."""
+    need_gpu()
+    w = Workload("mrg-pipes", "mrg32k3a", 12345, 260, 2**76, 203, dtype)
+    want, wst = oracle_run(w)
+    for hook in (None, "1"):
+        if hook:
+            monkeypatch.setenv("PRAND_MRG_INT", hook)
+        got, st, _ = lib_run(w, calls=[100, 103])
+        assert_same(w, got, want)
+        assert st == wst
+    monkeypatch.delenv("PRAND_MRG_INT", raising=False)
+
+
 def got_dtype(dtype):
     return {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
 
