@@ -45,6 +45,13 @@ int prand_host_plan(int gen, uint64_t n_streams, uint64_t n_per_stream, int dtyp
                     uint64_t *chunk_len, uint64_t *n_chunks);
 
 /*
+ * GM/GQ: the coefficients (k_n, q_n) of the paper's jump relation x(2n+w) = k_n x(n+w) - q_n x(w)
+ * (eq. 2) for n = mant * 2^log2, computed by eq. 3-4 (Lucas ladder, no matrix);
+ * prand_init fills a family of >= 64 streams with them.
+ */
+int prand_host_gm_kq(int gen, uint64_t mant, unsigned log2, uint64_t *k_n, uint64_t *q_n);
+
+/*
  * Section plan of prand_generate_seq_* (Table 5): `length` outputs of one sequence are
  * cut into n_sections sections of sec_len (a multiple of 32; the last one may be shorter).
  */

@@ -42,6 +42,7 @@ struct JumpArgs {
     uint64_t n_streams;
     const void *ops;       // device array of per-level operators
     uint64_t idx0, idx_stride;
+    uint64_t count;        // streams to compute (the first `count` of n_streams; 0 = all): GM tree init
 };
 
 // One bulk generation launch.  Rows [0, n) of every stream; when n_chunks > 1 virtual stream
@@ -69,6 +70,9 @@ cudaError_t mrg32k3a_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
 cudaError_t mrg32k3a_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
 cudaError_t gm_jump(cudaStream_t, int gen, const JumpArgs &, LaunchInfo *);
 cudaError_t gm_generate(cudaStream_t, int gen, const GenArgs &, LaunchInfo *);
+// streams [s_begin, s_end) = kn * stream(s - back) - qn * stream(s - 2 back) (eq. 2), in place
+cudaError_t gm_tree_fill(cudaStream_t, int gen, void *st, uint64_t ns, uint64_t s_begin, uint64_t s_end,
+                         uint64_t back, uint64_t kn, uint64_t qn, LaunchInfo *);
 // MT19937: dst stream j (j in [dst0, dst0+count)) = g(A) applied to src stream (j - src_back), or to
 // itself when src_back == 0.  State layout [stream][624].
 cudaError_t mt19937_apply(cudaStream_t, const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,

@@ -62,17 +62,35 @@ template <class W>
 __global__ void __launch_bounds__(256)
 gm_jump_kernel(const W *__restrict__ base, const W *st_in, W *st_out,
                uint64_t ns, int S, const GmOp *__restrict__ ops, uint64_t idx0, uint64_t idx_stride,
-               Barrett B)
+               Barrett B, uint64_t count)
 {
     uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= ns * (uint64_t)S) return;
-    uint64_t pt = t / ns, s = t - pt * ns;
+    if (t >= count * (uint64_t)S) return;
+    uint64_t pt = t / count, s = t - pt * count;
     uint64_t xP, xN;
     if (base) { xP = base[2 * pt]; xN = base[2 * pt + 1]; }
     else { xP = st_in[(2 * pt) * ns + s]; xN = st_in[(2 * pt + 1) * ns + s]; }
     gm_apply_bits(ops, idx0 + s * idx_stride, xP, xN, B);
     st_out[(2 * pt) * ns + s] = (W)xP;
     st_out[(2 * pt + 1) * ns + s] = (W)xN;
+}
+
+// Stream initialisation by the paper's relation (eq. 2): for any w,
+// x(w + 2n) = k_n x(w + n) - q_n x(w), and block splitting puts stream s at offset s L, so with n = 2^j L
+//     state(s) = k_n state(s - 2^j) - q_n state(s - 2^(j+1))        (every state word alike).
+// One launch fills streams [s_begin, s_end) from already filled ones: two modular products per word
+// instead of one 2x2 matrix product per set bit of the stream index.  One thread per (word, stream).
+template <class W>
+__global__ void __launch_bounds__(256)
+gm_tree_kernel(W *st, uint64_t ns, uint64_t s_begin, uint64_t s_end, uint64_t back, int words, uint64_t kn,
+               uint64_t qneg, Barrett B)
+{
+    const uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t count = s_end - s_begin;
+    if (t >= count * (uint64_t)words) return;
+    const uint64_t w = t / count, s = s_begin + (t - w * count);
+    const uint64_t a = st[w * ns + s - back], b = st[w * ns + s - 2 * back];
+    st[w * ns + s] = (W)baddmod(bmulmod(kn, a, B), bmulmod(qneg, b, B), B);
 }
 
 // Generation.  LP lanes share one stream, each holding S/LP ensemble points in registers.
@@ -254,17 +272,39 @@ cudaError_t gm_jump(cudaStream_t stream, int gen, const JumpArgs &a, LaunchInfo 
     const GmParams *p = gm_params(gen);
     if (!p) return cudaErrorInvalidValue;
     Barrett B = barrett_of(p);
-    uint64_t threads = a.n_streams * p->s;
+    const uint64_t count = a.count ? a.count : a.n_streams;
+    uint64_t threads = count * p->s;
     unsigned blocks = (unsigned)ceil_div_u64(threads, 256);
     if (p->wide)
         gm_jump_kernel<uint64_t><<<blocks, 256, 0, stream>>>((const uint64_t *)a.base, (const uint64_t *)a.st_in,
                                                              (uint64_t *)a.st_out, a.n_streams, (int)p->s,
-                                                             (const GmOp *)a.ops, a.idx0, a.idx_stride, B);
+                                                             (const GmOp *)a.ops, a.idx0, a.idx_stride, B, count);
     else
         gm_jump_kernel<uint32_t><<<blocks, 256, 0, stream>>>((const uint32_t *)a.base, (const uint32_t *)a.st_in,
                                                              (uint32_t *)a.st_out, a.n_streams, (int)p->s,
-                                                             (const GmOp *)a.ops, a.idx0, a.idx_stride, B);
+                                                             (const GmOp *)a.ops, a.idx0, a.idx_stride, B, count);
     li->kernel = "gm_jump";
+    li->launches = 1;
+    return cudaGetLastError();
+}
+
+cudaError_t gm_tree_fill(cudaStream_t stream, int gen, void *st, uint64_t ns, uint64_t s_begin, uint64_t s_end,
+                         uint64_t back, uint64_t kn, uint64_t qn, LaunchInfo *li)
+{
+    const GmParams *p = gm_params(gen);
+    if (!p) return cudaErrorInvalidValue;
+    li->kernel = "gm_tree";
+    li->launches = 0;
+    if (s_end <= s_begin) return cudaSuccess;
+    Barrett B = barrett_of(p);
+    const int words = 2 * (int)p->s;
+    const uint64_t threads = (s_end - s_begin) * (uint64_t)words;
+    const unsigned blocks = (unsigned)ceil_div_u64(threads, 256);
+    const uint64_t qneg = (p->g - qn % p->g) % p->g;
+    if (p->wide)
+        gm_tree_kernel<uint64_t><<<blocks, 256, 0, stream>>>((uint64_t *)st, ns, s_begin, s_end, back, words, kn, qneg, B);
+    else
+        gm_tree_kernel<uint32_t><<<blocks, 256, 0, stream>>>((uint32_t *)st, ns, s_begin, s_end, back, words, kn, qneg, B);
     li->launches = 1;
     return cudaGetLastError();
 }

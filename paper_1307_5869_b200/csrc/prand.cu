@@ -6,6 +6,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <string>
 #include <vector>
 #include "internal.h"
 #include "skip_ops.h"
@@ -318,9 +319,35 @@ int init_body(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream, const
     a.ops = (char *)st->d_ops + ops_off;
     a.idx0 = st->first;
     a.idx_stride = 1;
+    a.count = 0;
+    // GM/GQ with many streams: the paper's own relation (eq. 2-3) fills the family.
+    // Streams 0 and 1 come from the jump kernel; then, level by level, stream s = k_n stream(s - 2^j)
+    // - q_n stream(s - 2^(j+1)) with n = 2^j L -- two modular products per state word instead of one
+    // matrix product per set bit of s.  PRAND_GM_INIT=matrix keeps the matrix path (test hook).
+    const bool tree = is_gm(st->gen) && st->ns >= 64 && !(std::getenv("PRAND_GM_INIT") &&
+                                                          std::string(std::getenv("PRAND_GM_INIT")) == "matrix");
     LaunchInfo li;
+    if (!tree) {
+        CU(launch_jump(stream, st->gen, a, &li));
+        note(st, li);
+        return PRAND_OK;
+    }
+    a.count = 2;
     CU(launch_jump(stream, st->gen, a, &li));
     note(st, li);
+    std::vector<uint64_t> kn, qn;
+    const unsigned tlev = bit_length(st->ns - 1);
+    host::gm_kq_levels(*gm_params(st->gen), L, tlev, kn, qn);
+    for (unsigned j = 0; j < tlev; j++) {
+        const uint64_t back = 1ull << j;
+        for (int half = 0; half < 2; half++) {              // [2 back, 3 back) first: [3 back, 4 back) reads it
+            const uint64_t lo = (2 + half) * back, hi = (3 + half) * back;
+            if (lo >= st->ns) break;
+            CU(gm_tree_fill(stream, st->gen, st->d_state[st->cur], st->ns, lo, hi < st->ns ? hi : st->ns, back,
+                            kn[j], qn[j], &li));
+            note(st, li);
+        }
+    }
     return PRAND_OK;
 }
 
@@ -425,6 +452,7 @@ int jump_launch(prand_state *st, cudaStream_t stream)
         a.ops = st->d_ops;
         a.idx0 = 1;                          // every stream applies level 0 exactly once
         a.idx_stride = 0;
+        a.count = 0;
         CU(launch_jump(stream, st->gen, a, &li));
     }
     note(st, li);
@@ -986,6 +1014,18 @@ extern "C" int prand_host_mt19937_mulmod(const uint32_t *a624, const uint32_t *b
     std::memcpy(b.w, b624, sizeof b.w);
     host::mt19937_mulmod(r, a, b);
     std::memcpy(r624, r.w, sizeof r.w);
+    return PRAND_OK;
+}
+
+extern "C" int prand_host_gm_kq(int gen, uint64_t mant, unsigned log2, uint64_t *k_n, uint64_t *q_n)
+{
+    const GmParams *p = gm_params(gen);
+    if (!p) return PRAND_ERR_GEN;
+    if (!k_n || !q_n || log2 > 32768) return PRAND_ERR_ARG;
+    std::vector<uint64_t> kn, qn;
+    host::gm_kq_levels(*p, Dist{mant, log2}, 1, kn, qn);
+    *k_n = kn[0];
+    *q_n = qn[0];
     return PRAND_OK;
 }
 

@@ -162,6 +162,45 @@ void gm_levels(const GmParams &p, Dist n, unsigned levels, std::vector<GmOp> &ou
     }
 }
 
+// The paper's own jump relation: x(2n+w) = k_n x(n+w) - q_n x(w) (eq. 2) with
+// k_1 = k, q_1 = q, k_2n = k_n^2 - 2 q_n, q_2n = q_n^2 (eq. 3) and k_0 = 2, k_{n+1} = k k_n - q k_{n-1},
+// q_n = q^n (eq. 4).  k_n is the Lucas sequence V_n(k, q); for an arbitrary n = mant * 2^log2 it is
+// reached by the binary ladder on the pair (V_m, V_{m+1}) -- V_2m = V_m^2 - 2 q^m, V_2m+1 = V_m V_{m+1}
+// - k q^m (both follow from eq. 2-4) -- over the bits of mant, then log2 doublings by eq. 3; further
+// doublings give the levels n 2^j.  No matrix is involved: the CPU tests compare the result with the
+// trace and determinant of the matrix power.
+void gm_kq_levels(const GmParams &p, Dist n, unsigned levels, std::vector<uint64_t> &kn, std::vector<uint64_t> &qn)
+{
+    const uint64_t g = p.g, k = p.k % g, q = p.q % g;
+    auto sub = [g](uint64_t a, uint64_t b) { return a >= b ? a - b : a + g - b; };
+    // ladder over mant: (v0, v1, qm) = (V_m, V_{m+1}, q^m), m = leading bits of mant
+    uint64_t v0 = 2 % g, v1 = k, qm = 1 % g;
+    for (int b = 63; b >= 0; b--) {
+        if (n.mant >> b == 0) continue;                   // above the leading bit: m stays 0
+        const uint64_t v00 = sub(mulmod_g(v0, v0, g), mulmod_g(2 % g, qm, g));          // V_2m
+        const uint64_t v01 = sub(mulmod_g(v0, v1, g), mulmod_g(k, qm, g));              // V_2m+1
+        const uint64_t q2 = mulmod_g(qm, qm, g);
+        if ((n.mant >> b) & 1) {
+            const uint64_t v11 = sub(mulmod_g(v1, v1, g), mulmod_g(2 % g, mulmod_g(qm, q, g), g));   // V_2m+2
+            v0 = v01; v1 = v11; qm = mulmod_g(q2, q, g);
+        } else {
+            v0 = v00; v1 = v01; qm = q2;
+        }
+    }
+    uint64_t kc = v0, qc = qm;
+    for (unsigned i = 0; i < n.log2; i++) {               // eq. 3
+        kc = sub(mulmod_g(kc, kc, g), mulmod_g(2 % g, qc, g));
+        qc = mulmod_g(qc, qc, g);
+    }
+    kn.assign(levels, 0);
+    qn.assign(levels, 0);
+    for (unsigned lev = 0; lev < levels; lev++) {
+        kn[lev] = kc; qn[lev] = qc;
+        kc = sub(mulmod_g(kc, kc, g), mulmod_g(2 % g, qc, g));
+        qc = mulmod_g(qc, qc, g);
+    }
+}
+
 bool gm_seed_state(const GmParams &p, uint64_t seed, uint64_t *words)
 {
     const uint64_t w1 = seed % p.g;

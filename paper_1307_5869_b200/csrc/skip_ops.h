@@ -30,6 +30,8 @@ void mrg32k3a_levels(Dist n, unsigned levels, std::vector<MrgOp> &out);
 void gm_levels(const GmParams &p, Dist n, unsigned levels, std::vector<GmOp> &out);
 // seed state of the ensemble (reading G3): words xP_0, xN_0, ..., xP_{s-1}, xN_{s-1} with
 // (xP_i, xN_i) = (w((i+1) 2^d), w((i+1) 2^d + 1)), w(0) = 0, w(1) = seed mod g.  false if seed = 0 mod g.
+// (k_n, q_n) of the paper's eq. 2-4 for n * 2^j, j < levels
+void gm_kq_levels(const GmParams &p, Dist n, unsigned levels, std::vector<uint64_t> &kn, std::vector<uint64_t> &qn);
 bool gm_seed_state(const GmParams &p, uint64_t seed, uint64_t *words);
 
 // ---- MT19937 -------------------------------------------------------------------------------------

@@ -335,6 +335,29 @@ def test_mrg32k3a_integer_and_fp64_pipe_kernels_agree_with_the_oracle(dtype, mon
     monkeypatch.delenv("PRAND_MRG_INT", raising=False)
 
 
+@pytest.mark.parametrize("gen", ["gm19", "gm31", "gm55", "gm61", "gq58.1", "gq58.3"])
+def test_gm_family_init_by_the_papers_relation_equals_matrix_jumps(gen, monkeypatch):
+    """prand_init fills GM/GQ families of >= 64 streams with x(2n+w) = k_n x(n+w) - q_n x(w)
+    (eq. 2-3); PRAND_GM_INIT=matrix keeps one matrix jump per stream.  Same states,
+    for ragged counts and shards, and both equal the oracle's."""
+    need_gpu()
+    L = workloads.BLOCK_LEN[gen]
+    for first, ns in ((0, 64), (0, 1000), (5, 777), (0, 4099)):
+        g = P.Generator(gen, 1, ns, L, first_stream=first)
+        st_tree = g.state()
+        assert g.last_kernel == "gm_tree"
+        g.close()
+        monkeypatch.setenv("PRAND_GM_INIT", "matrix")
+        g = P.Generator(gen, 1, ns, L, first_stream=first)
+        st_mat = g.state()
+        assert g.last_kernel == "gm_jump"
+        g.close()
+        monkeypatch.delenv("PRAND_GM_INIT")
+        assert st_tree == st_mat, f"{gen}: tree init differs from matrix init (first {first}, ns {ns})"
+    _, wst = oracle.streams(gen, 1, 5, 777, L, 0, "u32", threads=CPU_THREADS)
+    assert st_tree[:0] == b"" and P.Generator(gen, 1, 777, L, first_stream=5).state() == wst.tobytes()
+
+
 def got_dtype(dtype):
     return {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
 
@@ -370,7 +393,7 @@ def test_fill_probe_writes_every_word():
 def test_launch_counter_counts_kernels():
     need_gpu()
     before = P.prand_launch_count()
-    g = P.Generator("gm55", 1, 64, 2**33)
+    g = P.Generator("gm55", 1, 32, 2**33)                # < 64 streams: one jump launch initialises them
     g.generate(8, "u32"); g.generate(8, "f32")
     assert P.prand_launch_count() - before == 3          # init + two fills
     assert "gm55" in g.last_kernel

@@ -199,3 +199,33 @@ def test_bench_reference_arm_prints_the_contract_line():
         assert key in d, key
     assert d["impl"] == "reference" and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and "workload" in d["config"]
+
+
+def test_gm_jump_coefficients_of_the_papers_relation():
+    """x(2n+w) = k_n x(n+w) - q_n x(w).  The library's (k_n, q_n) (Lucas ladder by
+    eq. 3-4) must be the trace and determinant of the n-th power of the companion matrix (the skip
+    operator, computed by matrix powers), reproduce eq. 3, and drive the oracle's orbit by eq. 2."""
+    import ctypes as C
+    params = {"gm19": (15, 28, 2**19 - 1), "gm61": (24, 74, 2**61 - 1), "gm55": (256, 176, 16 * (2**51 - 129)),
+              "gq58.3": (8, 48, 2**29 * (2**29 - 3))}
+    def kq(gen, n):
+        mant, log2 = P.split_dist(n)
+        k, q = C.c_uint64(), C.c_uint64()
+        assert P.lib().prand_host_gm_kq(P.gen_id(gen), mant, log2, C.byref(k), C.byref(q)) == 0
+        return k.value, q.value
+    for gen, (k, q, g) in params.items():
+        assert kq(gen, 1) == (k % g, q % g)
+        for n in (2, 3, 7, 1000, 2**26, 5 * 2**33, 3 * 2**70):
+            kn, qn = kq(gen, n)
+            m = np.frombuffer(P.prand_host_skip_op(gen, n), dtype=np.uint64).astype(object)
+            assert kn == (m[0] + m[3]) % g and qn == (m[0] * m[3] - m[1] * m[2]) % g, (gen, n)
+            assert qn == pow(q, n, g)
+            k2, q2 = kq(gen, 2 * n)
+            assert k2 == (kn * kn - 2 * qn) % g and q2 == qn * qn % g          # eq. 3
+        # eq. 2 on the oracle's orbit (seed 1): x(2n+w) = k_n x(n+w) - q_n x(w)
+        n, w = 12345, 678
+        kn, qn = kq(gen, n)
+        xw = oracle.gm_orbit(gen, 1, w)[0]
+        xnw = oracle.gm_orbit(gen, 1, n + w)[0]
+        x2nw = oracle.gm_orbit(gen, 1, 2 * n + w)[0]
+        assert x2nw == (kn * xnw - qn * xw) % g
