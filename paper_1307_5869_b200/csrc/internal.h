@@ -68,6 +68,9 @@ cudaError_t lfsr113_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
 cudaError_t lfsr113_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
 cudaError_t mrg32k3a_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
 cudaError_t mrg32k3a_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
+// sections of one sequence written in PRAND's contiguous layout (sec_len a multiple of 16, out 16-byte aligned)
+cudaError_t mrg32k3a_seq_f64(cudaStream_t, const void *st_in, double *out, uint64_t n_sections, uint64_t sec_len,
+                             uint64_t length, LaunchInfo *);
 cudaError_t gm_jump(cudaStream_t, int gen, const JumpArgs &, LaunchInfo *);
 cudaError_t gm_generate(cudaStream_t, int gen, const GenArgs &, LaunchInfo *);
 // streams [s_begin, s_end) = kn * stream(s - back) - qn * stream(s - 2 back) (eq. 2), in place

@@ -310,6 +310,62 @@ mrg32k3a_gen_fp64y_kernel(const uint32_t *st_in, uint32_t *st_out,
     }
 }
 
+// ---- sections of a single sequence, float64 (prand_generate_seq_f64; the paper's Table 7 task) -------
+// Thread t owns sections 2t and 2t+1 (as in the bulk kernel) but the array layout is PRAND's
+// contiguous one, out[c * sec_len + i].  A warp collects 16 rows of its 64 sections in a
+// shared-memory tile and writes them section by section: eight lanes store the 128 contiguous bytes of
+// one section's 16 numbers, so a warp store covers four full 128-byte lines.
+constexpr int SEQ_ROWS = 16, SEQ_PITCH = 17;               // tile[section][row], pitch in doubles
+
+__global__ void __launch_bounds__(GEN_THREADS)
+mrg32k3a_seq_f64_kernel(const uint32_t *st_in, double *__restrict__ out, uint64_t n_sections, uint64_t sec_len,
+                        uint64_t length)
+{
+    __shared__ double tile_all[GEN_THREADS / 32][64 * SEQ_PITCH];
+    double *tile = tile_all[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const uint64_t warp_sec0 = ((uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u)) * 2;   // first section of the warp
+    if (warp_sec0 >= n_sections) return;                   // whole warp
+    const uint64_t s0 = warp_sec0 + 2 * lane;
+    Mrg g[2];
+#pragma unroll
+    for (int v = 0; v < 2; v++) g[v] = mrg_load(st_in, n_sections, s0 + v < n_sections ? s0 + v : n_sections - 1);
+    uint32_t c1 = C1;
+    asm volatile("" : "+r"(c1));
+    // rows of the warp's sections: sec_len for all but the last section of the array
+    const uint64_t last = n_sections - 1;
+    const uint64_t last_rows = length - last * sec_len;
+#pragma unroll 1
+    for (uint64_t i0 = 0; i0 < sec_len; i0 += SEQ_ROWS) {
+#pragma unroll
+        for (int r = 0; r < SEQ_ROWS; r++) {
+#pragma unroll
+            for (int v = 0; v < 2; v++) {
+                const uint32_t nx = mrg_next_x(g[v].x1, g[v].x2, c1), ny = mrg_next_y(g[v].y0, g[v].y2);
+                g[v].x2 = g[v].x1; g[v].x1 = g[v].x0; g[v].x0 = nx;
+                g[v].y2 = g[v].y1; g[v].y1 = g[v].y0; g[v].y0 = ny;
+                tile[(2 * lane + v) * SEQ_PITCH + r] = mrg_output<DT_F64>(nx, ny);
+            }
+        }
+        __syncwarp();
+        const int sub = lane >> 3, piece = lane & 7;
+#pragma unroll 4
+        for (int k = 0; k < 16; k++) {
+            const int sl = 4 * k + sub;                    // section within the warp
+            const uint64_t sec = warp_sec0 + sl;
+            const uint64_t row = i0 + 2 * piece;
+            if (sec < n_sections) {
+                const uint64_t rows = sec == last ? last_rows : sec_len;
+                const double a = tile[sl * SEQ_PITCH + 2 * piece], b = tile[sl * SEQ_PITCH + 2 * piece + 1];
+                double *dst = out + sec * sec_len + row;
+                if (row + 1 < rows) store2(dst, a, b);
+                else if (row < rows) store1(dst, a);
+            }
+        }
+        __syncwarp();
+    }
+}
+
 template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
 {
     typedef typename OutElem<DT>::type T;
@@ -346,6 +402,17 @@ cudaError_t mrg32k3a_jump(cudaStream_t stream, const JumpArgs &a, LaunchInfo *li
                                                      (uint32_t *)a.st_out, a.n_streams,
                                                      (const MrgOp *)a.ops, a.idx0, a.idx_stride);
     li->kernel = "mrg32k3a_jump";
+    li->launches = 1;
+    return cudaGetLastError();
+}
+
+cudaError_t mrg32k3a_seq_f64(cudaStream_t stream, const void *st_in, double *out, uint64_t n_sections,
+                             uint64_t sec_len, uint64_t length, LaunchInfo *li)
+{
+    const uint64_t threads = ceil_div_u64(n_sections, 2);
+    mrg32k3a_seq_f64_kernel<<<(unsigned)ceil_div_u64(threads, GEN_THREADS), GEN_THREADS, 0, stream>>>(
+        (const uint32_t *)st_in, out, n_sections, sec_len, length);
+    li->kernel = "mrg32k3a_seq_f64";
     li->launches = 1;
     return cudaGetLastError();
 }

@@ -723,6 +723,13 @@ int generate_seq(prand_state *st, void *out, uint64_t length, int dtype, cudaStr
     Dist Ld = {L, 0};
     int rc = init_body(c, 0, Ld, stream, st->d_state[st->cur]);
     if (rc) return rc;
+    if (st->gen == PRAND_MRG32K3A && dtype == DT_F64 && (uintptr_t)out % 16 == 0) {
+        // fused path: the sections are written in place, no scratch buffer, no transposition
+        LaunchInfo li;
+        CU(mrg32k3a_seq_f64(stream, c->d_state[c->cur], (double *)out, S, L, length, &li));
+        note(st, li);
+        return prand_jump(st, length, 0, stream);
+    }
     void *tmp = nullptr;
     CU(dev_alloc(&tmp, (size_t)L * S * esz, stream));
     rc = generate(c, tmp, L, dtype, stream);
