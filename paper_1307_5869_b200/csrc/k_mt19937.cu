@@ -28,7 +28,6 @@ __device__ __forceinline__ uint32_t mt_recur(uint32_t xi, uint32_t xi1, uint32_t
 // set positions in shared memory, so that the accumulation loop has no bit scan and runs eight
 // positions (24 independent shared loads per thread) at a time; the list is padded with a position
 // whose words are zero.
-constexpr int APPLY_THREADS = 256;
 constexpr int APPLY_XWORDS = DEG + NW;                      // 20561
 constexpr int APPLY_ZERO = APPLY_XWORDS;                    // x[APPLY_ZERO .. +APPLY_ZPAD) = 0
 constexpr int APPLY_ZPAD = 771;                             // >= 768, makes the list 16-byte aligned
@@ -36,29 +35,45 @@ constexpr int APPLY_CHUNK = 64;                             // polynomial words 
 constexpr int APPLY_LIST = APPLY_CHUNK * 32 + 8;            // positions (u16) incl. padding
 constexpr size_t APPLY_SMEM = (size_t)(APPLY_XWORDS + APPLY_ZPAD) * sizeof(uint32_t) + APPLY_LIST * sizeof(uint16_t) + 16;
 
-__global__ void __launch_bounds__(APPLY_THREADS)
+// NT = 256: three output words per thread, two CTAs per SM (throughput: many streams); NT = 640: one
+// output word per thread, a third of the loads per thread (latency: the first levels of a doubling tree
+// and other launches with fewer CTAs than SMs).
+// SPLIT > 1: SPLIT CTAs share one application, each extending the window itself (cheap) and
+// accumulating 624 / SPLIT of the output words -- for launches with far fewer applications than SMs
+// (the first levels of a doubling tree), where the time of a level is the latency of one application.
+// Only for src != dst streams (src_back != 0): the parts of one stream run concurrently.
+template <int NT, int SPLIT>
+__global__ void __launch_bounds__(NT)
 mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
                      uint64_t src_back, const MtOp *__restrict__ op)
 {
+    constexpr int APPLY_THREADS = NT, NOUT = NW / SPLIT, NO = (NOUT + NT - 1) / NT;
+    static_assert(NW % SPLIT == 0, "SPLIT must divide 624");
+    const int out0 = (int)(blockIdx.x % SPLIT) * NOUT;
     extern __shared__ __align__(16) uint32_t smem[];
     uint32_t *x = smem;                                                      // APPLY_XWORDS + APPLY_ZPAD
     uint16_t *list = reinterpret_cast<uint16_t *>(smem + APPLY_XWORDS + APPLY_ZPAD);  // APPLY_LIST
     int *meta = reinterpret_cast<int *>(list + APPLY_LIST);                  // [0] warp-0 total, [1] count
     const int tid = threadIdx.x;
-    const uint64_t dst = dst0 + blockIdx.x;
+    const uint64_t dst = dst0 + blockIdx.x / SPLIT;
     const uint32_t *src = st_src + (dst - src_back) * NW;
     for (int j = tid; j < NW; j += APPLY_THREADS) x[j] = src[j];
     for (int j = tid; j < APPLY_ZPAD; j += APPLY_THREADS) x[APPLY_ZERO + j] = 0;
     __syncthreads();
-    for (int r0 = 0; r0 < DEG; r0 += 227) {
+    constexpr int EXT = NT < NW - MW ? NT : NW - MW;       // at most 227 new words are independent
+    for (int r0 = 0; r0 < DEG; r0 += EXT) {
         int k = r0 + tid;
-        if (tid < 227 && k < DEG) x[NW + k] = mt_recur(x[k], x[k + 1], x[k + MW]);
+        if (tid < EXT && k < DEG) x[NW + k] = mt_recur(x[k], x[k + 1], x[k + MW]);
         __syncthreads();
     }
-    // thread t accumulates output words t, t+256, t+512 (the last only for t < 112)
-    uint32_t acc0 = 0, acc1 = 0, acc2 = 0;
-    const uint32_t *x0 = x + tid, *x1 = x + tid + 256;
-    const uint32_t *x2 = x + (tid + 512 < NW ? tid + 512 : 0);
+    // thread t accumulates output words t, t + NT, ... (those below 624)
+    uint32_t acc[NO];
+    const uint32_t *xo[NO];
+#pragma unroll
+    for (int o = 0; o < NO; o++) {
+        acc[o] = 0;
+        xo[o] = x + (tid + NT * o < NOUT ? out0 + tid + NT * o : 0);
+    }
     for (int c0 = 0; c0 < NW; c0 += APPLY_CHUNK) {
         // expand polynomial words c0 .. c0+63 (threads 0..63, two warps) into the list of set positions
         if (tid < APPLY_CHUNK) {
@@ -91,17 +106,18 @@ mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
 #pragma unroll
             for (int h = 0; h < 4; h++) {
                 const int ia = ii[h] & 0xFFFF, ib = ii[h] >> 16;
-                acc0 ^= x0[ia] ^ x0[ib];
-                acc1 ^= x1[ia] ^ x1[ib];
-                acc2 ^= x2[ia] ^ x2[ib];
+#pragma unroll
+                for (int o = 0; o < NO; o++) acc[o] ^= xo[o][ia] ^ xo[o][ib];
             }
         }
         __syncthreads();
     }
     uint32_t *d = st_dst + dst * NW;
-    d[tid] = tid == 0 ? (acc0 & 0x80000000u) : acc0;   // only the top bit of word 0 is state (T2)
-    d[tid + 256] = acc1;
-    if (tid + 512 < NW) d[tid + 512] = acc2;
+#pragma unroll
+    for (int o = 0; o < NO; o++) {
+        const int j = out0 + tid + NT * o;
+        if (tid + NT * o < NOUT) d[j] = j == 0 ? (acc[o] & 0x80000000u) : acc[o];   // only the top bit of word 0 is state (T2)
+    }
 }
 
 // ---- generation ----------------------------------------------------------------------------------
@@ -528,8 +544,14 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
 {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(mt19937_apply_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(mt19937_apply_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)APPLY_SMEM);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(mt19937_apply_kernel<640, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)APPLY_SMEM);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(mt19937_apply_kernel<160, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)APPLY_SMEM);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -537,7 +559,13 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
     li->launches = 0;
     // grid.x is limited to 2^31-1 blocks; streams beyond that would not fit device memory anyway
     if (count == 0) return cudaSuccess;
-    mt19937_apply_kernel<<<(unsigned)count, APPLY_THREADS, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+    // fewer CTAs than SMs: the launch is as long as one application
+    if (src_back != 0 && 4 * count <= 2 * (uint64_t)sm_count())
+        mt19937_apply_kernel<160, 4><<<(unsigned)(4 * count), 160, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+    else if (count <= (uint64_t)sm_count())
+        mt19937_apply_kernel<640, 1><<<(unsigned)count, 640, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+    else
+        mt19937_apply_kernel<256, 1><<<(unsigned)count, 256, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     li->launches = 1;
     return cudaGetLastError();
 }
