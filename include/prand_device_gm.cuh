@@ -48,6 +48,8 @@ template <> struct Gm<PRAND_GM19> {
     __device__ static __forceinline__ void pack(uint32_t &word, R x, const int J) { word = pack_mad(word, x >> 18, J); }
 };
 
+static __constant__ uint32_t gm29_c[3] = {0u - 2u, 2u * ((1u << 29) - 3), 4u};
+
 template <> struct Gm<PRAND_GM29> {
     typedef uint32_t W;
     typedef uint32_t R;
@@ -58,8 +60,10 @@ template <> struct Gm<PRAND_GM29> {
     __device__ static __forceinline__ W store(R x) { return x; }
     __device__ static __forceinline__ R step(R xP, R xN)
     {
-        uint32_t t = xP * (0u - 2u) + 2u * G;
-        t = xN * 4u + t;                                   // < 6 g < 2^32
+        // multipliers from constant memory: two IMADs (as literals the compiler turns them into three
+        // shift/add instructions)
+        uint32_t t = xP * gm29_c[0] + gm29_c[1];           // 2 (g - xP)
+        t = xN * gm29_c[2] + t;                            // + 4 xN < 6 g < 2^32
         uint32_t r = (t >> 29) * (0u - G) + t;             // 2^29 = 3 (mod g): (t & (2^29-1)) + 3 (t >> 29) < 2^29 + 15
         return umin_sub(r, G);
     }
