@@ -120,6 +120,69 @@ mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
     }
 }
 
+// Throughput form of the same application (many destination streams).  Thread t accumulates the four
+// consecutive output words 4t .. 4t+3.  For the 32 coefficients of one polynomial word pw (positions
+// 32 wi + b) they read x[32 wi + 4t + b + c], c < 4: a window of 35 consecutive words, loaded as nine
+// aligned 16-byte shared loads into registers; bit b of pw (the same for all threads) then predicates
+// four register XORs.  36 words loaded per 64 XORs on average instead of one load per XOR.
+constexpr int APPLYW_THREADS = 160;                         // 156 active in the accumulation
+
+__global__ void __launch_bounds__(APPLYW_THREADS)
+mt19937_apply_win_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
+                         uint64_t src_back, const MtOp *__restrict__ op)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    uint32_t *x = smem;                                    // APPLY_XWORDS + APPLY_ZPAD
+    const int tid = threadIdx.x;
+    const uint64_t dst = dst0 + blockIdx.x;
+    const uint32_t *src = st_src + (dst - src_back) * NW;
+    for (int j = tid; j < NW; j += APPLYW_THREADS) x[j] = src[j];
+    for (int j = tid; j < APPLY_ZPAD; j += APPLYW_THREADS) x[APPLY_ZERO + j] = 0;
+    __syncthreads();
+    for (int r0 = 0; r0 < DEG; r0 += APPLYW_THREADS) {
+        int k = r0 + tid;
+        if (k < DEG) x[NW + k] = mt_recur(x[k], x[k + 1], x[k + MW]);
+        __syncthreads();
+    }
+    if (tid >= NW / 4) return;
+    uint32_t acc[4][4] = {};                               // four interleaved sets: independent XOR chains
+    const uint4 *xw = reinterpret_cast<const uint4 *>(x) + tid;   // window of wi starts at xw[8 wi]
+    // two register windows in ping-pong: the nine loads of the next polynomial word are issued before
+    // the 128 predicated XORs of the current one
+    uint4 wa[9], wb[9];
+    auto load_win = [&](uint4 (&w)[9], int wi) {
+#pragma unroll
+        for (int q = 0; q < 9; q++) w[q] = xw[8 * wi + q];
+    };
+    auto accumulate = [&](const uint4 (&w)[9], uint32_t pw) {
+        uint32_t v[36];
+#pragma unroll
+        for (int q = 0; q < 9; q++) { v[4 * q] = w[q].x; v[4 * q + 1] = w[q].y; v[4 * q + 2] = w[q].z; v[4 * q + 3] = w[q].w; }
+#pragma unroll
+        for (int b = 0; b < 32; b++) {
+            if (pw & (1u << b)) {
+                acc[b & 3][0] ^= v[b]; acc[b & 3][1] ^= v[b + 1]; acc[b & 3][2] ^= v[b + 2]; acc[b & 3][3] ^= v[b + 3];
+            }
+        }
+    };
+    load_win(wa, 0);
+    uint32_t pw0 = __ldg(&op->w[0]), pw1 = __ldg(&op->w[1]);
+#pragma unroll 1
+    for (int wi = 0; wi < NW; wi += 2) {
+        load_win(wb, wi + 1);
+        const uint32_t p0 = pw0, p1 = pw1;
+        if (wi + 2 < NW) { pw0 = __ldg(&op->w[wi + 2]); pw1 = __ldg(&op->w[wi + 3]); }
+        accumulate(wa, p0);
+        load_win(wa, wi + 2 < NW ? wi + 2 : wi);
+        accumulate(wb, p1);
+    }
+    uint32_t *d = st_dst + dst * NW + 4 * tid;
+    uint32_t r[4];
+#pragma unroll
+    for (int c = 0; c < 4; c++) r[c] = acc[0][c] ^ acc[1][c] ^ acc[2][c] ^ acc[3][c];
+    *reinterpret_cast<uint4 *>(d) = make_uint4(tid == 0 ? (r[0] & 0x80000000u) : r[0], r[1], r[2], r[3]);
+}
+
 // ---- generation ----------------------------------------------------------------------------------
 // CTA = S adjacent streams x T word slices (thread = (slice t, stream ls), ls fastest).  Thread
 // (t, ls) owns the K = 624/T words w = T j + t, j = 0..K-1, of stream ls and keeps them in registers.
@@ -552,6 +615,9 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
         if (e == cudaSuccess)
             e = cudaFuncSetAttribute(mt19937_apply_kernel<160, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      (int)APPLY_SMEM);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(mt19937_apply_win_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)APPLY_SMEM);
         if (e != cudaSuccess) return e;
         attr_set = true;
     }
@@ -564,8 +630,10 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
         mt19937_apply_kernel<160, 4><<<(unsigned)(4 * count), 160, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     else if (count <= (uint64_t)sm_count())
         mt19937_apply_kernel<640, 1><<<(unsigned)count, 640, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    else
+    else if (std::getenv("PRAND_MT_APPLY_LIST"))             // test hook: the position-list kernel at any size
         mt19937_apply_kernel<256, 1><<<(unsigned)count, 256, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+    else
+        mt19937_apply_win_kernel<<<(unsigned)count, APPLYW_THREADS, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     li->launches = 1;
     return cudaGetLastError();
 }
