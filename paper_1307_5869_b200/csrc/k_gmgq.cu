@@ -228,6 +228,116 @@ gm_gen_kernel(const typename Tr::W *st_in, typename Tr::W *st_out,
     }
 }
 
+// ---- GM31: some of the 32 points on the FP64 pipe ----------------------------------------------------
+// The integer step of GM31 is bound by the FMA-heavy pipe (two half-rate 32x32+64 multiply-adds per
+// point) while the FP64 pipe (64 lanes/clk/SM) idles.  NF of the 32 points are therefore kept as
+// doubles and stepped there, exactly (g = 2^31 - 1):
+//   p = 11 xN + 14 (g - xP) in [0, 25 * 2^31)       two DFMA, integers below 2^36: exact
+//   k = floor(p / g) = rint(p * (1/g) - 0.5 + 2^-33)   p/g is an integer or at least 1/g = 2^-31 away from
+//                                                   one, the product is off by < 2^-47: the rounding can
+//                                                   never go the wrong way; rint as +- 1.5 * 2^52
+//   x' = p - k g in [0, g)                          one DFMA, exact and already canonical
+// The digit (bit 30) is read from the low mantissa word of x' + 1.5 * 2^52.  Seven FP64 instructions,
+// one shift and one multiply-add per point, against four ALU and six FMA-pipe slots for the integer
+// step; with NF = 14 the three pipes are about evenly loaded.
+template <int NF, int DT>
+__global__ void __launch_bounds__(128)
+gm31_hybrid_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT>::type *__restrict__ out,
+                   uint64_t ns, uint64_t n, uint64_t chunk_len, uint64_t n_chunks,
+                   const GmOp *__restrict__ chunk_ops, Barrett B)
+{
+    typedef Gm<PRAND_GM31> Tr;
+    typedef typename OutElem<DT>::type T;
+    constexpr int NI = 32 - NF;
+    constexpr double GD = 2147483647.0, MAGIC = 6755399441055744.0;
+    const uint64_t vs = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = vs < ns * n_chunks;
+    const uint64_t c = valid ? vs / ns : 0, s = valid ? vs - c * ns : 0;
+    double dA[NF], dB[NF];                                  // points 0 .. NF-1
+    uint32_t iA[NI], iB[NI];                                // points NF .. 31
+#pragma unroll
+    for (int j = 0; j < 32; j++) {
+        uint32_t a = valid ? st_in[(uint64_t)(2 * j) * ns + s] : 0u;
+        uint32_t b = valid ? st_in[(uint64_t)(2 * j + 1) * ns + s] : 0u;
+        if (c != 0) {
+            uint64_t a64 = a, b64 = b;
+            gm_apply_bits(chunk_ops + (c - 1), 1, a64, b64, B);
+            a = (uint32_t)a64; b = (uint32_t)b64;
+        }
+        if (j < NF) { dA[j] = (double)a; dB[j] = (double)b; }
+        else { iA[j - NF] = a; iB[j - NF] = b; }
+    }
+    const uint64_t row0 = valid ? c * chunk_len : 0;
+    const uint64_t row1 = valid ? ((row0 + chunk_len < n) ? row0 + chunk_len : n) : 0;
+
+    auto step_d = [&](double xP, double xN, uint32_t &word, const int j) -> double {
+        const double t = __fma_rn(-14.0, xP, 14.0 * GD);
+        const double p = __fma_rn(11.0, xN, t);
+        const double sq = __fma_rn(p, 4.6566128752457969e-10, -0.5 + 1.1641532182693481e-10);   // 1/g, 2^-33
+        const double kk = __dadd_rn(__dadd_rn(sq, MAGIC), -MAGIC);
+        const double r = __fma_rn(-kk, GD, p);
+        const uint32_t v = (uint32_t)__double2loint(__dadd_rn(r, MAGIC));
+        word = pack_mad(word, v >> 30, j);
+        return r;
+    };
+    // PAR = false: (A, B) = (x(n-1), x(n)) and A receives x(n+1); PAR = true: roles swapped
+    auto step_word = [&](auto par) -> uint32_t {
+        constexpr bool PAR = decltype(par)::value;
+        uint32_t word = 0;
+#pragma unroll
+        for (int j = 0; j < 32; j++) {
+            if (j < NF) {
+                const int q = j < NF ? j : 0;
+                if (!PAR) dA[q] = step_d(dA[q], dB[q], word, j); else dB[q] = step_d(dB[q], dA[q], word, j);
+            } else {
+                const int q = j >= NF ? j - NF : 0;
+                if (!PAR) { iA[q] = Tr::step(iA[q], iB[q]); Tr::pack(word, iA[q], j); }
+                else { iB[q] = Tr::step(iB[q], iA[q]); Tr::pack(word, iB[q], j); }
+            }
+        }
+        return word;
+    };
+    T *p = out + row0 * ns + s;
+    uint64_t i = row0;
+    bool odd = false;
+#pragma unroll 1
+    for (; i + 2 <= row1; i += 2) {
+        store1(p, convert<DT>(step_word(std::false_type())));
+        p += ns;
+        store1(p, convert<DT>(step_word(std::true_type())));
+        p += ns;
+    }
+    if (i < row1) {
+        store1(p, convert<DT>(step_word(std::false_type())));
+        odd = true;
+    }
+    if (valid && c == n_chunks - 1) {
+#pragma unroll
+        for (int j = 0; j < 32; j++) {
+            uint32_t a, b;
+            if (j < NF) { a = (uint32_t)__double2uint_rn(dA[j < NF ? j : 0]); b = (uint32_t)__double2uint_rn(dB[j < NF ? j : 0]); }
+            else { a = iA[j >= NF ? j - NF : 0]; b = iB[j >= NF ? j - NF : 0]; }
+            st_out[(uint64_t)(2 * j) * ns + s] = odd ? b : a;
+            st_out[(uint64_t)(2 * j + 1) * ns + s] = odd ? a : b;
+        }
+    }
+}
+
+template <int NF> cudaError_t launch_gm31_hybrid(cudaStream_t stream, const GenArgs &a, const Barrett &B)
+{
+    const uint64_t lanes = a.n_streams * a.n_chunks;
+    const unsigned blocks = (unsigned)ceil_div_u64(lanes, 128);
+    const uint32_t *si = (const uint32_t *)a.st_in;
+    uint32_t *so = (uint32_t *)a.st_out;
+    const GmOp *co = (const GmOp *)a.chunk_ops;
+    switch (a.dtype) {
+    case DT_U32: gm31_hybrid_kernel<NF, DT_U32><<<blocks, 128, 0, stream>>>(si, so, (uint32_t *)a.out, a.n_streams, a.n, a.chunk_len, a.n_chunks, co, B); break;
+    case DT_F32: gm31_hybrid_kernel<NF, DT_F32><<<blocks, 128, 0, stream>>>(si, so, (float *)a.out, a.n_streams, a.n, a.chunk_len, a.n_chunks, co, B); break;
+    default: gm31_hybrid_kernel<NF, DT_F64><<<blocks, 128, 0, stream>>>(si, so, (double *)a.out, a.n_streams, a.n, a.chunk_len, a.n_chunks, co, B); break;
+    }
+    return cudaGetLastError();
+}
+
 // Limit of the optimistic steps' watch value (Tr::WATCH_LIMIT); the test hook PRAND_GM_WATCH lowers it
 // so that the exact fallback runs often (0: always).
 template <class Tr> uint32_t gm_watch_limit()
@@ -320,7 +430,15 @@ cudaError_t gm_generate(cudaStream_t stream, int gen, const GenArgs &a, LaunchIn
     switch (gen) {
     case PRAND_GM19: li->kernel = "gm19_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM19>, 1>(stream, a, B);
     case PRAND_GM29: li->kernel = "gm29_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM29>, 1>(stream, a, B);
-    case PRAND_GM31: li->kernel = "gm31_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM31>, 1>(stream, a, B);
+    case PRAND_GM31: {
+        int nf = 14;                                         // points on the FP64 pipe (test / tuning hook)
+        if (const char *env = std::getenv("PRAND_GM31_NF")) nf = std::atoi(env);
+        if (nf == 12) { li->kernel = "gm31_gen<fp64 x12>"; return launch_gm31_hybrid<12>(stream, a, B); }
+        if (nf == 14) { li->kernel = "gm31_gen<fp64 x14>"; return launch_gm31_hybrid<14>(stream, a, B); }
+        if (nf == 16) { li->kernel = "gm31_gen<fp64 x16>"; return launch_gm31_hybrid<16>(stream, a, B); }
+        if (nf == 10) { li->kernel = "gm31_gen<fp64 x10>"; return launch_gm31_hybrid<10>(stream, a, B); }
+        li->kernel = "gm31_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM31>, 1>(stream, a, B);
+    }
     case PRAND_GM61:
         if (lp == 1) { li->kernel = "gm61_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM61>, 1, 2>(stream, a, B); }
         if (lp == 2) { li->kernel = "gm61_gen<LP=2>"; return dispatch_dt<Gm<PRAND_GM61>, 2>(stream, a, B); }

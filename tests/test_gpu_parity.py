@@ -358,6 +358,21 @@ def test_gm_family_init_by_the_papers_relation_equals_matrix_jumps(gen, monkeypa
     assert st_tree[:0] == b"" and P.Generator(gen, 1, 777, L, first_stream=5).state() == wst.tobytes()
 
 
+@pytest.mark.parametrize("nf", ["0", "10", "16"])
+def test_gm31_points_on_the_fp64_pipe_are_exact(nf, monkeypatch):
+    """GM31 steps 14 of its 32 points in double precision on the FP64 pipe (exact floor division by
+    2^31 - 1); PRAND_GM31_NF selects other splits (0: all points on the integer pipes)."""
+    need_gpu()
+    monkeypatch.setenv("PRAND_GM31_NF", nf)
+    w = Workload("gm31-fp64", "gm31", 1, 300, workloads.BLOCK_LEN["gm31"], 101, "u32")
+    got, st, kernel = lib_run(w, calls=[50, 51])
+    want, wst = oracle_run(w)
+    assert_same(w, got, want)
+    assert st == wst
+    assert ("fp64" in kernel) == (nf != "0")
+    monkeypatch.delenv("PRAND_GM31_NF")
+
+
 def got_dtype(dtype):
     return {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
 
