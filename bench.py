@@ -45,7 +45,7 @@ ARITH = {"lfsr113": "u32", "mrg32k3a": "u32 (32x32->64 mul, mod 2^32-c) + f64 sc
 # Integer-bound generators (DESIGN.md 6.4/6.5): thread-instructions per number of the generation loop
 # (SASS counts of the committed kernels, confirmed by ncu smsp__inst_executed in profiles/r01b_summary.md)
 # against the issue peak 148 SMs x 4 schedulers x 32 lanes x sm_max_mhz.
-ALU_INSTR_PER_NUMBER = {"gm19": 250, "gm29": 263, "gm31": 266, "gm61": 545, "gm55": 195, "gq58.1": 306,
+ALU_INSTR_PER_NUMBER = {"gm19": 250, "gm29": 263, "gm31": 285, "gm61": 545, "gm55": 195, "gq58.1": 306,
                         "gq58.3": 148, "gq58.4": 103}
 
 
