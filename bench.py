@@ -18,6 +18,10 @@ block_len 2^76, 16,384 float64 per stream = 2^30 numbers, 8 GiB).  Prints ONE JS
              same run is reported beside it
   cpu_baseline  the CPU oracle, as it stands, on all host cores, on a bounded sample of the workload
 
+  per_config every other BASELINE.json configuration (C1, C3, C4 x2, C5 x9) and the paper's Table 7 task
+             (T7 x2), generation call alone: gen_ms, Gnumbers/s, bound, frac, kernel, init_ms, clocks; plus
+             launch_floor_us (empty kernel) and memset_write_peak_gbs (N = 1 only)
+
 ``--impl reference`` times the oracle alone (this tier's reference arm).  ``--gpus N`` under torchrun
 shards the block-split family by stream index (weak scaling, no data-path collective).
 """
@@ -42,11 +46,32 @@ UNIT = "Gnumbers/s"
 ARITH = {"lfsr113": "u32", "mrg32k3a": "u32 (32x32->64 mul, mod 2^32-c) + f64 scale", "mt19937": "u32"}
 
 
-# Integer-bound generators (DESIGN.md 6.4/6.5): thread-instructions per number of the generation loop
-# (SASS counts of the committed kernels, confirmed by ncu smsp__inst_executed in profiles/r01b_summary.md)
-# against the issue peak 148 SMs x 4 schedulers x 32 lanes x sm_max_mhz.
-ALU_INSTR_PER_NUMBER = {"gm19": 250, "gm29": 263, "gm31": 285, "gm61": 545, "gm55": 195, "gq58.1": 306,
-                        "gq58.3": 148, "gq58.4": 103}
+# State bytes per stream: read once and written once per generate call.
+STATE_BYTES = {"lfsr113": 16, "mrg32k3a": 24, "mt19937": 2496, "gm19": 256, "gm29": 256, "gm31": 256,
+               "gm55": 128, "gm61": 512, "gq58.1": 512, "gq58.3": 192, "gq58.4": 128}
+ALU_BOUND = {"gm19", "gm29", "gm31", "gm55", "gm61", "gq58.1", "gq58.3", "gq58.4"}
+
+
+def load_alu_counts():
+    """Thread-instructions per number of the integer-bound generation kernels, as counted by ncu
+    (smsp__inst_executed.sum x 32 / numbers) in the committed --set full captures: profiles/alu_counts.csv
+    is written from those captures (its `source` column names the details file), never edited by hand."""
+    import csv
+    path = os.path.join(ROOT, "profiles", "alu_counts.csv")
+    out = {}
+    if os.path.exists(path):
+        with open(path, newline="") as f:
+            for row in csv.DictReader(f):
+                out[row["kernel"]] = (float(row["thread_instr_per_number"]), row["source"])
+    return out
+
+
+def algorithmic_bytes(w):
+    """output element + state read and write-back amortised over n_per_stream; a
+    single-sequence fill (T7) counts its output only."""
+    if w.seq:
+        return w.out_bytes
+    return w.out_bytes + 2 * STATE_BYTES[w.gen] * w.n_streams
 
 
 def alu_peak_ginstr():
@@ -170,7 +195,9 @@ def run_reference(args, w):
     value = statistics.mean(rates)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": wall / max(1, args.steps) * 1e3,
+        "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": w.numbers / (value * 1e9) * 1e3,      # a full step of `config` at the sampled rate
+        "sample_wall_ms_per_step": wall / max(1, args.steps) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": ARITH.get(w.gen, "u32/u64 modular"), "data": "synthetic",
         "config": config_of(w),
@@ -192,6 +219,110 @@ def config_of(w):
 
 
 # ---- our arm -----------------------------------------------------------------------------------------
+def roofline_of(w, kernel, k_ms, peak, peak_src, share=None, fill_gbs=None):
+    """The bench line's `roofline` object for one launch of `kernel` that took k_ms on workload w."""
+    alg = algorithmic_bytes(w)
+    out_gbs = w.out_bytes / (k_ms * 1e-3) / 1e9
+    alg_gbs = alg / (k_ms * 1e-3) / 1e9
+    traffic = load_traffic(kernel)
+    if w.gen in ALU_BOUND:                         # integer-bound: report against the issue peak
+        counts = load_alu_counts()
+        ipn, src = counts.get(kernel, (None, None))
+        p_g = alu_peak_ginstr()
+        a_g = ipn * w.numbers / (k_ms * 1e-3) / 1e9 if ipn else None
+        r = {"bound": "alu", "achieved": a_g, "peak": p_g, "unit": "Gthread-instr/s",
+             "frac": a_g / p_g if a_g else None, "traffic": traffic, "kernel": kernel, "kernel_ms": k_ms,
+             "thread_instr_per_number": ipn, "thread_instr_source": src,
+             "peak_source": "148 SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md 6.5, profiles/pipe_rates.md)",
+             "out_gbs": out_gbs, "hbm_peak_gbs": peak, "frac_of_hbm": alg_gbs / peak}
+    else:
+        r = {"bound": "hbm", "achieved": alg_gbs, "peak": peak, "unit": "GB/s", "frac": alg_gbs / peak,
+             "traffic": traffic, "kernel": kernel, "kernel_ms": k_ms,
+             "algorithmic_bytes_per_launch": alg, "out_bytes_per_launch": w.out_bytes, "out_gbs": out_gbs,
+             "peak_source": peak_src}
+        if fill_gbs:
+            r["write_peak_same_run_gbs"] = fill_gbs
+            r["frac_of_write_peak"] = alg_gbs / fill_gbs
+    if share is not None:
+        r["kernel_share_of_step"] = share
+    return r
+
+
+def event_ms(torch, fn, n, warm=3, before=None):
+    """CUDA-event durations (ms) of n calls of fn on torch's current stream, each after `before()`."""
+    out = []
+    for i in range(warm + n):
+        if before:
+            before()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); fn(); b.record()
+        torch.cuda.synchronize()
+        if i >= warm:
+            out.append(a.elapsed_time(b))
+    return out
+
+
+def write_peaks(torch, P, nbytes=2 << 30):
+    """Write roofline of this run: the fill probe (128-bit st.global.cs of a constant) and cudaMemsetAsync."""
+    buf = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    fill = event_ms(torch, lambda: P.prand_fill_u32(buf.data_ptr(), nbytes // 4, 0x12345678), 10)
+    mset = event_ms(torch, lambda: P.prand_probe_memset(buf.data_ptr(), 0x5A, nbytes), 10)
+    del buf
+    return nbytes / (statistics.median(fill) * 1e-3) / 1e9, nbytes / (statistics.median(mset) * 1e-3) / 1e9
+
+
+def launch_floor_us(torch, P):
+    """Empty kernel on the same stream: event-to-event time of one launch (what a small configuration's
+    event pair measures at least), and the per-launch time of 1000 back-to-back launches."""
+    single = event_ms(torch, P.prand_probe_empty, 200, warm=20)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record()
+    for _ in range(1000):
+        P.prand_probe_empty()
+    b.record()
+    torch.cuda.synchronize()
+    return {"single_event_pair_us_median": statistics.median(single) * 1e3,
+            "single_event_pair_us_min": min(single) * 1e3,
+            "back_to_back_us_per_launch": a.elapsed_time(b)}
+
+
+def time_config(torch, P, w, steps, warmup, flush, peak, peak_src, device_index=0):
+    """One per_config row: stream initialisation (wall clock around prand_init + synchronise, host
+    operator preparation included) and the generation call alone (CUDA events, L2 flushed before each)."""
+    tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[w.dtype]
+    name = ("prand_generate_seq_" if w.seq else "prand_generate_") + w.dtype
+    out = torch.empty((w.n_per_stream, w.n_streams), dtype=tdt, device="cuda")
+    init_ms, h = [], None
+    for _ in range(3):
+        if h:
+            P.prand_free(h)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        h = P.prand_init(w.gen, w.seed, w.n_streams, w.block_len)
+        torch.cuda.synchronize()
+        init_ms.append((time.perf_counter() - t0) * 1e3)
+    l0 = P.prand_launch_count()
+    with ClockSampler(device_index) as clk:
+        gen_ms = event_ms(torch, lambda: P._generate(name, h, out.data_ptr(), w.n_per_stream, None), steps,
+                          warm=warmup, before=flush.zero_)
+    launches = (P.prand_launch_count() - l0) // (steps + warmup)
+    kernel = P.prand_last_kernel(h)
+    P.prand_free(h)
+    del out
+    torch.cuda.empty_cache()
+    med = statistics.median(gen_ms)
+    roof = roofline_of(w, kernel, med, peak, peak_src)
+    return {"workload": w.name, "gen": w.gen, "dtype": w.dtype, "n_streams": w.n_streams,
+            "n_per_stream": w.n_per_stream, "api": name, "kernel": kernel, "launches_per_call": launches,
+            "gen_ms": med, "gen_ms_best": min(gen_ms), "gnumbers_per_s": w.numbers / (med * 1e-3) / 1e9,
+            "bound": roof["bound"], "frac": roof["frac"], "out_gbs": roof["out_gbs"],
+            "algorithmic_bytes": algorithmic_bytes(w), "frac_of_hbm": roof.get("frac_of_hbm", roof["frac"]),
+            "thread_instr_per_number": roof.get("thread_instr_per_number"),
+            "init_ms": min(init_ms), "init_streams_per_s": w.n_streams / (min(init_ms) * 1e-3),
+            "clocks": clk.summary()}
+
+
 def run_ours(args, w):
     import torch
     import paper_1307_5869_b200 as P
@@ -222,7 +353,7 @@ def run_ours(args, w):
     first, _ = sharding.weak_shard(w.n_streams, rank)   # weak scaling: rank r holds streams [r ns, (r+1) ns)
     out = torch.empty((w.n_per_stream, w.n_streams), dtype=tdt, device="cuda")
     need_flush = w.out_bytes <= (1 << 30)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if need_flush else None
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     last_kernel = [""]
 
     def step(ev=None):
@@ -263,17 +394,11 @@ def run_ours(args, w):
     ms_per_step = elapsed_ms / args.steps
     value = world * w.numbers / (ms_per_step * 1e-3) / 1e9
 
-    # write peak of the same run (fill probe, same buffer)
-    fill_ms = []
-    for i in range(13):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        P.prand_fill_u32(out.data_ptr(), w.out_bytes // 4, 0x12345678)
-        b.record()
-        torch.cuda.synchronize()
-        if i >= 3:
-            fill_ms.append(a.elapsed_time(b))
+    # write peak of the same run: fill probe on the same buffer, cudaMemsetAsync as the second opinion
+    fill_ms = event_ms(torch, lambda: P.prand_fill_u32(out.data_ptr(), w.out_bytes // 4, 0x12345678), 10)
+    mset_ms = event_ms(torch, lambda: P.prand_probe_memset(out.data_ptr(), 0x5A, w.out_bytes), 10)
     fill_gbs = w.out_bytes / (statistics.median(fill_ms) * 1e-3) / 1e9
+    memset_gbs = w.out_bytes / (statistics.median(mset_ms) * 1e-3) / 1e9
 
     # end to end through the host-delivery entry point
     e2e = None
@@ -305,6 +430,7 @@ def run_ours(args, w):
                "d2h_bytes_per_step": w.out_bytes, "steps": ke, "warmup": 1, "ms_per_step": ev_ms / ke,
                "api": f"prand_generate_{w.dtype}_host (pinned host buffer)"}
         del host
+    del out
 
     if rank != 0:
         if dist is not None:
@@ -312,22 +438,8 @@ def run_ours(args, w):
         return
     peak, peak_src = load_peaks()
     k_ms = statistics.mean(kernel_ms)
-    achieved = w.out_bytes / (k_ms * 1e-3) / 1e9
-    traffic = load_traffic(last_kernel[0])
-    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "kernel": last_kernel[0], "kernel_ms": k_ms,
-                "kernel_share_of_step": k_ms / ms_per_step,
-                "algorithmic_bytes_per_launch": w.out_bytes, "peak_source": peak_src,
-                "write_peak_same_run_gbs": fill_gbs, "frac_of_write_peak": achieved / fill_gbs}
-    if w.gen in ALU_INSTR_PER_NUMBER:              # integer-bound: report against the issue peak
-        ipn = ALU_INSTR_PER_NUMBER[w.gen]
-        a_g = ipn * w.numbers / (k_ms * 1e-3) / 1e9
-        p_g = alu_peak_ginstr()
-        roofline = {"bound": "alu", "achieved": a_g, "peak": p_g, "unit": "Gthread-instr/s", "frac": a_g / p_g,
-                    "traffic": traffic, "kernel": last_kernel[0], "kernel_ms": k_ms,
-                    "kernel_share_of_step": k_ms / ms_per_step, "thread_instr_per_number": ipn,
-                    "peak_source": "148 SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md 6.5)",
-                    "out_gbs": achieved, "hbm_peak_gbs": peak}
+    roofline = roofline_of(w, last_kernel[0], k_ms, peak, peak_src, share=k_ms / ms_per_step, fill_gbs=fill_gbs)
+    roofline["memset_write_peak_gbs"] = memset_gbs
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -335,7 +447,23 @@ def run_ours(args, w):
         "config": config_of(w),
         "roofline": roofline,
         "e2e": e2e, "gpu_launches": launches, "clocks": clk.summary(),
+        "write_peak_gbs": fill_gbs, "memset_write_peak_gbs": memset_gbs,
     }
+    if world == 1 and not args.no_per_config:
+        # every other configuration of BASELINE.json (+ the paper's Table 7 task), generation call alone
+        torch.cuda.empty_cache()
+        line["launch_floor_us"] = launch_floor_us(torch, P)
+        rows = []
+        for name in workloads.ALL:
+            rows.append(time_config(torch, P, workloads.ALL[name], args.config_steps, 3, flush, peak, peak_src,
+                                    local_rank))
+            print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
+        line["per_config"] = rows
+        line["per_config_note"] = ("generation call alone (prand_generate_* / prand_generate_seq_*), CUDA-event median of "
+                                   f"{args.config_steps} calls after 3 warm-ups, 256 MB written before each call (L2 flush); "
+                                   "frac: hbm = algorithmic bytes (output + 2 x state) / gen_ms / MEASURED_PEAKS hbm_gbs; "
+                                   "alu = ncu thread-instructions per number (profiles/alu_counts.csv) x numbers / gen_ms / "
+                                   "issue peak; init_ms = best wall time of prand_init + synchronise (3 runs)")
     if world == 1 and not args.no_cpu:
         import oracle
         oracle.build()
@@ -353,65 +481,41 @@ def run_sweep(args):
     import paper_1307_5869_b200 as P
 
     torch.cuda.set_device(0)
-    peak, _ = load_peaks()
+    peak, peak_src = load_peaks()
     names = args.sweep_workloads.split(",") if args.sweep_workloads else list(workloads.ALL)
-    rows = []
-    fill_buf = torch.empty(2 << 30, dtype=torch.uint8, device="cuda")
-    fill_ms = []
-    for i in range(13):
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record(); P.prand_fill_u32(fill_buf.data_ptr(), fill_buf.numel() // 4, 1); b.record()
-        torch.cuda.synchronize()
-        if i >= 3:
-            fill_ms.append(a.elapsed_time(b))
-    fill_gbs = fill_buf.numel() / (statistics.median(fill_ms) * 1e-3) / 1e9
-    del fill_buf
+    fill_gbs, memset_gbs = write_peaks(torch, P)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    rows = []
     for name in names:
-        w = workloads.ALL[name]
-        tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[w.dtype]
-        gen_fn = {"u32": P.prand_generate_u32, "f32": P.prand_generate_f32, "f64": P.prand_generate_f64}[w.dtype]
-        if w.seq:
-            seq_name = "prand_generate_seq_" + w.dtype
-
-            def gen_fn(h, ptr, n, _name=seq_name):
-                P._generate(_name, h, ptr, n, None)
-        out = torch.empty((w.n_per_stream, w.n_streams), dtype=tdt, device="cuda")
-        init_ms = []
-        h = None
-        for i in range(3):
-            if h:
-                P.prand_free(h)
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            h = P.prand_init(w.gen, w.seed, w.n_streams, w.block_len)
-            torch.cuda.synchronize()
-            init_ms.append((time.perf_counter() - t0) * 1e3)
-        gen_ms = []
-        for i in range(args.warmup + args.steps):
-            flush.zero_()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(); gen_fn(h, out.data_ptr(), w.n_per_stream); b.record()
-            torch.cuda.synchronize()
-            if i >= args.warmup:
-                gen_ms.append(a.elapsed_time(b))
-        kernel = P.prand_last_kernel(h)
-        P.prand_free(h)
-        del out
-        torch.cuda.empty_cache()
-        med, best = statistics.median(gen_ms), min(gen_ms)
-        gbs = w.out_bytes / (med * 1e-3) / 1e9
-        row = {"workload": w.name, "gen": w.gen, "dtype": w.dtype, "n_streams": w.n_streams,
-               "n_per_stream": w.n_per_stream, "kernel": kernel, "gen_ms_median": med, "gen_ms_best": best,
-               "gnumbers_per_s": w.numbers / (med * 1e-3) / 1e9, "out_gbs": gbs, "frac_of_hbm_copy_peak": gbs / peak,
-               "frac_of_write_peak": gbs / fill_gbs, "init_ms_best": min(init_ms),
-               "init_streams_per_s": w.n_streams / (min(init_ms) * 1e-3)}
-        rows.append(row)
-        print(json.dumps(row), file=sys.stderr, flush=True)
-    result = {"write_peak_gbs": fill_gbs, "hbm_copy_peak_gbs": peak, "rows": rows}
+        rows.append(time_config(torch, P, workloads.ALL[name], args.steps, args.warmup, flush, peak, peak_src))
+        print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
+    result = {"write_peak_gbs": fill_gbs, "memset_write_peak_gbs": memset_gbs, "hbm_copy_peak_gbs": peak,
+              "launch_floor_us": launch_floor_us(torch, P), "rows": rows}
     with open(args.sweep, "w") as f:
         json.dump(result, f, indent=1)
     print(json.dumps({"sweep": args.sweep, "write_peak_gbs": fill_gbs, "n_rows": len(rows)}), flush=True)
+
+
+# ---- instruction rates of the SM pipes (profiles/pipe_rates.md) ----------------------------------------
+def run_pipe_rates(args):
+    import torch
+    import paper_1307_5869_b200 as P
+
+    torch.cuda.set_device(0)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    rows = []
+    for op, name in enumerate(P.prand_probe_pipe_names()):
+        ops = [0]
+
+        def fn(op=op):
+            ops[0] = P.prand_probe_pipe(op, 2000)
+        with ClockSampler(0, period_s=0.001) as clk:
+            ms = event_ms(torch, fn, 15, warm=3)
+        mhz = clk.summary()["sm_mhz"] or 1965.0
+        med = statistics.median(ms)
+        rows.append({"op": name, "ms": med, "thread_ops": ops[0], "sm_mhz": mhz,
+                     "ops_per_clk_per_sm": ops[0] / (med * 1e-3) / (mhz * 1e6) / sms})
+    print(json.dumps({"pipe_rates": rows, "sms": sms}), flush=True)
 
 
 def main():
@@ -425,10 +529,15 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--sweep", default=None, metavar="OUT.json", help="time every workload, write a table")
     ap.add_argument("--sweep-workloads", default=None, help="comma-separated workload names for --sweep")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config table (all other configs)")
+    ap.add_argument("--config-steps", type=int, default=10, help="timed calls per per_config row")
+    ap.add_argument("--pipe-rates", action="store_true", help="print the SM pipe instruction rates (probe kernels)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours" and not args.sweep:
         args.warmup = 3                          # timing rule: at least three warm-up steps
     w = workloads.ALL[args.workload]
+    if args.pipe_rates:
+        return run_pipe_rates(args)
     if args.sweep:
         return run_sweep(args)
     if args.impl == "reference":

@@ -194,6 +194,23 @@ int prand_free(prand_state *st);
  */
 int prand_fill_u32(uint32_t *out, uint64_t n_words, uint32_t value, void *cuda_stream);
 
+/*
+ * Measurement probes; none of them is on the hot path.
+ *   prand_probe_empty   launches an empty kernel (1 CTA x 32 threads) on `cuda_stream`: the launch floor
+ *                       that small configurations (C1) are compared with.
+ *   prand_probe_memset  cudaMemsetAsync of `bytes` at DEVICE pointer d_ptr: second opinion on the write peak.
+ *   prand_probe_pipe    launches the instruction-rate probe number `op` (0 .. prand_probe_pipe_count()-1,
+ *                       named by prand_probe_pipe_name) on 8 CTAs x 256 threads per SM; *thread_ops (HOST
+ *                       pointer) receives the thread-level operations one launch executes, so that
+ *                       thread_ops / (time x SM clock x SM count) = operations per clock per SM
+ *                       (profiles/pipe_rates.md).
+ */
+int prand_probe_empty(void *cuda_stream);
+int prand_probe_memset(void *d_ptr, int value, size_t bytes, void *cuda_stream);
+int prand_probe_pipe_count(void);
+const char *prand_probe_pipe_name(int op);
+int prand_probe_pipe(int op, uint64_t iters, uint64_t *thread_ops, void *cuda_stream);
+
 /* Number of kernels this library has launched in this process (for bench.py's gpu_launches). */
 uint64_t prand_launch_count(void);
 

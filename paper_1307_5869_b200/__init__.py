@@ -50,6 +50,11 @@ _SIGS = {
     "prand_generate_strided_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint, C.c_void_p]),
     "prand_free": (C.c_int, [C.c_void_p]),
     "prand_fill_u32": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p]),
+    "prand_probe_empty": (C.c_int, [C.c_void_p]),
+    "prand_probe_memset": (C.c_int, [C.c_void_p, C.c_int, C.c_size_t, C.c_void_p]),
+    "prand_probe_pipe_count": (C.c_int, []),
+    "prand_probe_pipe_name": (C.c_char_p, [C.c_int]),
+    "prand_probe_pipe": (C.c_int, [C.c_int, C.c_uint64, C.POINTER(C.c_uint64), C.c_void_p]),
     "prand_launch_count": (C.c_uint64, []),
     "prand_uploaded_bytes": (C.c_uint64, []),
     "prand_last_kernel": (C.c_char_p, [C.c_void_p]),
@@ -189,6 +194,25 @@ def prand_free(state: int) -> None:
 
 def prand_fill_u32(out_ptr: int, n_words: int, value: int, stream=None) -> None:
     _check(lib().prand_fill_u32(out_ptr, n_words, value, _stream_ptr(stream)), "prand_fill_u32")
+
+
+def prand_probe_empty(stream=None) -> None:
+    _check(lib().prand_probe_empty(_stream_ptr(stream)), "prand_probe_empty")
+
+
+def prand_probe_memset(ptr: int, value: int, nbytes: int, stream=None) -> None:
+    _check(lib().prand_probe_memset(ptr, value, nbytes, _stream_ptr(stream)), "prand_probe_memset")
+
+
+def prand_probe_pipe(op: int, iters: int, stream=None) -> int:
+    """Launch instruction-rate probe `op`; -> thread-level operations the launch executes."""
+    n = C.c_uint64()
+    _check(lib().prand_probe_pipe(op, iters, C.byref(n), _stream_ptr(stream)), "prand_probe_pipe")
+    return n.value
+
+
+def prand_probe_pipe_names() -> list[str]:
+    return [lib().prand_probe_pipe_name(i).decode() for i in range(lib().prand_probe_pipe_count())]
 
 
 def prand_launch_count() -> int:
