@@ -600,6 +600,342 @@ template <int HI> cudaError_t dispatch_bdt(cudaStream_t stream, const GenArgs &a
     }
 }
 
+// ---- generation, few streams: output gathered across a cluster of 4 CTAs ----------------------------
+// With a few hundred streams (C3: 512) a CTA can hold only ~4 of them, and a CTA that writes 16-byte
+// pieces of a row is bound by the SM's store path: measured 7.4 B/clk/SM for 16-byte pieces against
+// 17 B/clk/SM for 32-byte and ~21 B/clk/SM for 64-byte and longer ones (the request rate, about one
+// per two clocks, is what limits; TMA tensor stores of such narrow boxes are slower still).  So the
+// four CTAs of a cluster (16 adjacent streams) exchange their outputs through distributed shared
+// memory: CTA r computes the full recurrence of its own 4 streams, as above, but CTA d writes rows
+// [156 d, 156 d + 156) of every round (624 rows) for all 16 streams, i.e. 64-byte pieces, as 128-bit
+// stores.  Thread = (stream, word slice) with the stream index slowest: the threads of one stream meet
+// at their own named barrier, so the four streams of a CTA drift apart and fill each other's waits.
+//
+// Exchange: a round's numbers go to a local staging tile (one column per (destination, stream), 156
+// rows); a helper warp sends the 16 columns with bulk asynchronous copies (cp.async.bulk shared::cta ->
+// shared::cluster) that signal the destination's mbarrier by transaction bytes -- no release fence (a
+// cluster-scope fence is a MEMBAR.ALL.GPU, ~800 clocks per round when tried), no spinning on the data
+// path.  NB = 4 tile buffers, read-out LAG = 2 rounds behind: every wait has a full round of slack.
+//   full[b]   (count 1 + tx)  destination: all 16 columns of a tile have landed
+//   empty[b]  (count 4)       source: all four destinations have written tile b out (its staging and
+//                             gather buffers may be reused)
+//   prod[b] / cons[b] (count 28) local: the compute warps have staged / read tile b
+constexpr int CG_CS = 4, CG_S = 4;
+constexpr int CG_T = 208;                                 // words per wave (three waves per round)
+constexpr int CG_U = CG_T / 2;                            // a thread owns two adjacent words of a wave: 104 threads per stream
+constexpr int CG_GT = 128;                                // threads per group = one stream (104) rounded up to whole warps
+constexpr int CG_GROUPS = CG_S;
+constexpr int CG_COLS = CG_CS * CG_S;                     // streams per cluster
+constexpr int CG_ROWS = NW / CG_CS;                       // rows of a round written by one CTA
+constexpr int CG_CP = 192;                                // column pitch in words (768 B: a bulk copy)
+constexpr int CG_ROT = 2;                                 // column c starts CG_ROT * c words into its slot: conflict-free read-out
+constexpr int CG_NB = 4, CG_LAG = 2;
+constexpr int CG_P = 628;                                 // window pitch
+constexpr int CG_TILE = CG_COLS * CG_CP;                  // words per tile buffer
+constexpr int CG_CT = CG_GROUPS * CG_GT;                  // compute threads (448)
+constexpr int CG_WARPS = CG_CT / 32;                      // compute warps (14); the next warp is the helper
+constexpr int CG_THREADS = CG_CT + 32;
+constexpr int CG_PIECES = CG_ROWS * (CG_COLS / 4);        // 16-byte pieces of a gathered tile (624)
+constexpr uint32_t CG_TILE_BYTES = CG_TILE * 4;
+constexpr size_t CG_SMEM = (size_t)(2 * CG_S * CG_P + 2 * CG_NB * CG_TILE) * sizeof(uint32_t) + 4 * CG_NB * 8;
+static_assert(NW % CG_CS == 0 && CG_ROWS % 2 == 0 && CG_ROWS + CG_ROT * (CG_COLS - 1) <= CG_CP && CG_T * 3 == NW, "bad cluster tiling");
+static_assert(CG_LAG < CG_NB && (CG_NB & (CG_NB - 1)) == 0 && CG_CP % 4 == 0 && CG_P % 2 == 0 && CG_ROT % 2 == 0, "bad pipeline");
+
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t addr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void mbar_init(uint32_t a, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(a), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t a, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(a), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t a)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(a) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr)
+{
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" :: "r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t a, uint32_t parity)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+                 "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@!p bra WAIT_%=;\n\t}"
+                 :: "r"(a), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_to_cta(uint32_t dst_cluster, uint32_t src, uint32_t bytes, uint32_t mbar_cluster)
+{
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst_cluster), "r"(src), "r"(bytes), "r"(mbar_cluster) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void group_barrier(int g)
+{
+    asm volatile("bar.sync %0, %1;" :: "r"(1 + g), "n"(CG_GT) : "memory");
+}
+template <int DT> __device__ __forceinline__ uint32_t out_bits(uint32_t u)
+{
+    if constexpr (DT == DT_F32) return __float_as_uint(u32_to_f32(u));
+    else return u;
+}
+
+// One wave for one thread: words w = 208 J + 2u and w + 1 of its stream.  x_w, x_{w+1} are registers,
+// x_{w+2} and the two x_{w+397} (old window) resp. new x_{w-227} come from shared memory.  The cell after
+// the old window's last word holds the new word 0 (written in wave 0), so a pair never needs a special
+// case: for w <= 226 both operands are old[w + 397 ..] (old[624] = new[0]), else new[w - 227 ..].
+template <int J>
+__device__ __forceinline__ void cg_operands(const uint32_t *smem, const uint32_t ia, const uint32_t ib, const int u,
+                                            uint32_t &x2, uint32_t &m0, uint32_t &m1)
+{
+    x2 = smem[ia + CG_T * J + 2];
+    if (CG_T * (J + 1) <= NW - MW) { m0 = smem[ia + CG_T * J + MW]; m1 = smem[ia + CG_T * J + MW + 1]; }
+    else if (CG_T * J > NW - MW) { m0 = smem[ib + CG_T * J - (NW - MW)]; m1 = smem[ib + CG_T * J - (NW - MW) + 1]; }
+    else {
+        const uint32_t q = (CG_T * J + 2 * u <= NW - MW - 1 ? ia + MW : ib - (NW - MW)) + CG_T * J;
+        m0 = smem[q]; m1 = smem[q + 1];
+    }
+}
+// Full wave.  (p0, p1) carry the previous wave's two new words, whose tempering and staging store (slot
+// pend_slot of tile sb) run here, after this wave's loads have been issued, if `pending`.
+template <int J, int DT>
+__device__ __forceinline__ void cg_wave(uint32_t *smem, const uint32_t ia, const uint32_t ib, const int u,
+                                        uint32_t (&r)[6], const MtMul &c, uint32_t &p0, uint32_t &p1, uint32_t *sb,
+                                        const uint32_t pend_slot, const bool pending)
+{
+    uint32_t x2, m0, m1;
+    cg_operands<J>(smem, ia, ib, u, x2, m0, m1);
+    if (pending)
+        *reinterpret_cast<uint2 *>(sb + pend_slot) = make_uint2(out_bits<DT>(mt_temper2<0>(p0, c)), out_bits<DT>(mt_temper2<0>(p1, c)));
+    const uint32_t n0 = mt_recur2<0>(r[2 * J], r[2 * J + 1], m0, c);
+    const uint32_t n1 = mt_recur2<0>(r[2 * J + 1], x2, m1, c);
+    r[2 * J] = n0;
+    r[2 * J + 1] = n1;
+    *reinterpret_cast<uint2 *>(smem + ib + CG_T * J) = make_uint2(n0, n1);
+    if (J == 0 && u == 0) smem[ia + NW] = n0;
+    p0 = n0;
+    p1 = n1;
+}
+// Ragged tail: only words below `rem` are produced; (o0, o1) = the converted outputs.
+template <int J, int DT>
+__device__ __forceinline__ void cg_tail_wave(uint32_t *smem, const uint32_t ia, const uint32_t ib, const int u,
+                                             uint32_t (&r)[6], const MtMul &c, uint32_t &o0, uint32_t &o1, const int rem)
+{
+    const int w = CG_T * J + 2 * u;
+    if (w >= rem) return;
+    uint32_t x2, m0, m1;
+    cg_operands<J>(smem, ia, ib, u, x2, m0, m1);
+    const uint32_t n0 = mt_recur2<0>(r[2 * J], r[2 * J + 1], m0, c);
+    const uint32_t n1 = mt_recur2<0>(r[2 * J + 1], x2, m1, c);
+    smem[ib + CG_T * J] = n0;
+    if (w + 1 < rem) smem[ib + CG_T * J + 1] = n1;
+    if (J == 0 && u == 0) smem[ia + NW] = n0;
+    o0 = out_bits<DT>(mt_temper2<0>(n0, c));
+    o1 = out_bits<DT>(mt_temper2<0>(n1, c));
+}
+
+template <int DT>
+__global__ void __launch_bounds__(CG_THREADS)
+mt19937_cgen_kernel(const uint32_t *st_in, uint32_t *st_out, uint32_t *__restrict__ out, uint64_t ns, uint64_t n,
+                    const MtMul c)
+{
+    static_assert(DT == DT_U32 || DT == DT_F32, "4-byte outputs only");
+    extern __shared__ __align__(128) uint32_t smem[];    // windows [2][S][P], staging [NB][COLS][CP], gather [NB][COLS][CP], mbarriers
+    uint32_t *stage = smem + 2 * CG_S * CG_P;
+    uint32_t *gat = stage + CG_NB * CG_TILE;
+    const uint32_t bars = smem_addr(gat + CG_NB * CG_TILE);           // full, empty, prod, cons: [NB] each
+    const uint32_t full = bars, empty = bars + 8 * CG_NB, prod = bars + 16 * CG_NB, cons = bars + 24 * CG_NB;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const bool helper = tid >= CG_CT;
+    const int g = helper ? 0 : tid / CG_GT, tg = tid % CG_GT;         // group = stream within the CTA, thread in group
+    const bool act = !helper && tg < CG_U;
+    const int ls = g, u = act ? tg : 0;                               // word pair
+    uint32_t rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    const uint64_t sc0 = (uint64_t)(blockIdx.x / CG_CS) * CG_COLS;       // first stream of the cluster
+    const uint64_t s0 = sc0 + rank * CG_S;                                // first stream of this CTA
+    const uint64_t s = s0 + ls;
+    const bool live = s < ns;
+    const int n_live = s0 >= ns ? 0 : (ns - s0 < (uint64_t)CG_S ? (int)(ns - s0) : CG_S);
+    const uint32_t rounds = (uint32_t)(n / NW);           // the launcher keeps n / 624 below 2^32
+    const int rem = (int)(n % NW);
+
+    if (tid == 0) {
+        for (int b = 0; b < CG_NB; b++) {
+            mbar_init(full + 8 * b, 1);
+            mbar_init(empty + 8 * b, CG_CS);
+            mbar_init(prod + 8 * b, CG_WARPS);
+            mbar_init(cons + 8 * b, CG_WARPS);
+            if ((uint32_t)b < rounds) mbar_expect_tx(full + 8 * b, CG_TILE_BYTES);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = tid; i < CG_S * (NW / 4); i += CG_THREADS) {
+        const int q = i / (NW / 4), w4 = i % (NW / 4);
+        uint4 v = make_uint4(0u, 0u, 0u, 0u);
+        if (q < n_live) v = __ldg(reinterpret_cast<const uint4 *>(st_in + (s0 + q) * NW) + w4);
+        *reinterpret_cast<uint4 *>(smem + q * CG_P + 4 * w4) = v;
+    }
+    __syncthreads();
+    cluster_sync_all();                                   // every CTA's barriers are initialised
+    uint32_t ia = ls * CG_P + 2 * u, ib = ia + CG_S * CG_P;
+    const uint32_t cur = rounds & 1;                      // window buffer that is "old" after the full rounds
+    uint32_t r[6] = {0u, 0u, 0u, 0u, 0u, 0u};
+
+    if (helper) {
+        // ---- helper warp: forwards staged tiles, returns buffers -------------------------------------
+        const uint32_t copy_dst = map_to_cta(smem_addr(gat + (rank * CG_S + (lane & 3)) * CG_CP), (uint32_t)(lane >> 2) & 3u);
+        const uint32_t copy_bar = map_to_cta(full, (uint32_t)(lane >> 2) & 3u);
+        const uint32_t copy_src = smem_addr(stage + (lane & 15) * CG_CP);
+        const uint32_t free_bar = map_to_cta(empty, (uint32_t)lane & 3u);
+        for (uint32_t rd = 0; rd < rounds + CG_LAG; rd++) {
+            if (rd < rounds) {
+                const uint32_t b = rd & (CG_NB - 1), ph = (rd / CG_NB) & 1u;
+                mbar_wait(prod + 8 * b, ph);
+                // column (destination lane / 4, own stream lane % 4) -> column (rank, stream) of that CTA's tile
+                if (lane < CG_COLS)
+                    bulk_copy_to_cta(copy_dst + b * CG_TILE_BYTES, copy_src + b * CG_TILE_BYTES, CG_CP * 4, copy_bar + 8 * b);
+            }
+            if (rd >= CG_LAG) {
+                const uint32_t q = rd - CG_LAG;
+                const uint32_t b = q & (CG_NB - 1), ph = (q / CG_NB) & 1u;
+                mbar_wait(cons + 8 * b, ph);
+                if (lane == 0 && q + CG_NB < rounds) mbar_expect_tx(full + 8 * b, CG_TILE_BYTES);
+                __syncwarp();
+                if (lane < CG_CS) mbar_arrive_cluster(free_bar + 8 * b);
+            }
+        }
+    } else {
+        // ---- compute warps --------------------------------------------------------------------------------
+        if (act) {
+#pragma unroll
+            for (int j = 0; j < 3; j++) { r[2 * j] = smem[ia + CG_T * j]; r[2 * j + 1] = smem[ia + CG_T * j + 1]; }
+        }
+        // staging slots of this thread's words w = 208 j + 2u, w + 1: column (destination w / 156, own stream),
+        // rows w % 156 and the next one (same destination: 156 is even)
+        uint32_t so[3];
+#pragma unroll
+        for (int j = 0; j < 3; j++) {
+            const int w = CG_T * j + 2 * u;
+            so[j] = (uint32_t)(((w / CG_ROWS) * CG_S + ls) * CG_CP + CG_ROT * (rank * CG_S + ls) + w % CG_ROWS);
+        }
+        // read-out of a gathered tile: 156 rows x 16 streams as 624 pieces of 16 bytes, piece = (row, 4 streams);
+        // thread tid takes pieces tid and tid + CG_CT (the shared-memory pattern is conflict-free: 8 rows x 4 column
+        // groups per warp, column pitch = 2 mod 32)
+        constexpr int RO = (CG_PIECES + CG_CT - 1) / CG_CT;
+        uint32_t ro_src[RO];
+        uint64_t ro_dst[RO];
+        bool ro_on[RO];
+#pragma unroll
+        for (int k = 0; k < RO; k++) {
+            const int i = tid + k * CG_CT, row = i >> 2, cq = i & 3;
+            ro_on[k] = i < CG_PIECES && sc0 + 4 * cq < ns;
+            ro_src[k] = (uint32_t)((4 * cq) * (CG_CP + CG_ROT) + row);
+            ro_dst[k] = ((uint64_t)rank * CG_ROWS + row) * ns + sc0 + 4 * cq;
+        }
+        const uint64_t round_elems = (uint64_t)NW * ns;
+        uint32_t *ro_out = out;                           // row 0 of the next round to be read out
+        auto read_out = [&](uint32_t q) {
+            const uint32_t b = q & (CG_NB - 1), ph = (q / CG_NB) & 1u;
+            mbar_wait(full + 8 * b, ph);
+            const uint32_t *gb = gat + b * CG_TILE;
+#pragma unroll
+            for (int k = 0; k < RO; k++) {
+                if (ro_on[k]) {
+                    const uint32_t *gp = gb + ro_src[k];
+                    const uint4 v = make_uint4(gp[0], gp[CG_CP + CG_ROT], gp[2 * (CG_CP + CG_ROT)], gp[3 * (CG_CP + CG_ROT)]);
+                    __stcs(reinterpret_cast<uint4 *>(ro_out + ro_dst[k]), v);
+                }
+            }
+            ro_out += round_elems;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(cons + 8 * b);
+        };
+        // The tempering and the staging store of a wave's two numbers are deferred until the next wave's shared
+        // loads have been issued: after a barrier every warp of the group waits for shared memory at the same
+        // time, and the deferred half of the work is what fills that wait.
+        uint32_t p0 = 0, p1 = 0;
+        for (uint32_t rd = 0; rd < rounds; rd++) {
+            const uint32_t b = rd & (CG_NB - 1), ph = (rd / CG_NB) & 1u;
+            if (rd >= CG_NB) mbar_wait(empty + 8 * b, ph ^ 1u);           // tile rd - NB has been written out everywhere
+            uint32_t *sb = stage + b * CG_TILE;
+            if (act) cg_wave<0, DT>(smem, ia, ib, u, r, c, p0, p1, sb, 0u, false);
+            group_barrier(g);
+            if (act) cg_wave<1, DT>(smem, ia, ib, u, r, c, p0, p1, sb, so[0], true);
+            group_barrier(g);
+            if (act) cg_wave<2, DT>(smem, ia, ib, u, r, c, p0, p1, sb, so[1], true);
+            group_barrier(g);
+            if (act) *reinterpret_cast<uint2 *>(sb + so[2]) = make_uint2(out_bits<DT>(mt_temper2<0>(p0, c)), out_bits<DT>(mt_temper2<0>(p1, c)));
+            { const uint32_t tmp = ia; ia = ib; ib = tmp; }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");    // staged numbers -> visible to the bulk copy
+            __syncwarp();
+            if (lane == 0) mbar_arrive(prod + 8 * b);
+            if (rd >= CG_LAG) read_out(rd - CG_LAG);
+        }
+        for (uint32_t q = rounds > CG_LAG ? rounds - CG_LAG : 0; q < rounds; q++) read_out(q);
+    }
+    // nobody leaves while a peer may still send it a tile or a signal
+    cluster_sync_all();
+    // ragged tail (< 624 rows): straight to global memory
+    if (rem && !helper) {
+        uint32_t *p = out + (uint64_t)rounds * NW * ns + s;
+        uint32_t o0 = 0, o1 = 0;
+#define PRAND_CG_TAIL(J)                                                                      \
+        if (act) {                                                                            \
+            const int w = CG_T * J + 2 * u;                                                   \
+            cg_tail_wave<J, DT>(smem, ia, ib, u, r, c, o0, o1, rem);                         \
+            if (live && w < rem) __stcs(p + (uint64_t)w * ns, o0);                            \
+            if (live && w + 1 < rem) __stcs(p + (uint64_t)(w + 1) * ns, o1);                  \
+        }                                                                                     \
+        group_barrier(g);
+        PRAND_CG_TAIL(0)
+        PRAND_CG_TAIL(1)
+        PRAND_CG_TAIL(2)
+#undef PRAND_CG_TAIL
+    }
+    __syncthreads();
+    // final window x_{P+n}..x_{P+n+623}: words [rem, 624) of the old buffer, then [0, rem) of the new
+    const uint32_t *a0 = smem + cur * (CG_S * CG_P), *b0 = smem + (cur ^ 1) * (CG_S * CG_P);
+    for (int i = tid; i < CG_S * NW; i += CG_THREADS) {
+        const int q = i / NW, j = i % NW;
+        if (q < n_live) {
+            const int pp = j + rem;
+            st_out[(s0 + q) * NW + j] = pp < NW ? a0[q * CG_P + pp] : b0[q * CG_P + pp - NW];
+        }
+    }
+}
+
+template <int DT> cudaError_t launch_cgen(cudaStream_t stream, const GenArgs &a)
+{
+    auto kern = mt19937_cgen_kernel<DT>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)CG_SMEM);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(ceil_div_u64(a.n_streams, CG_COLS) * CG_CS));
+    cfg.blockDim = dim3(CG_THREADS);
+    cfg.dynamicSmemBytes = CG_SMEM;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = CG_CS;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const MtMul c = {2u * 0x1908B0DFu, 1u << 31, 1u << 21, 1u << 14};
+    return cudaLaunchKernelEx(&cfg, kern, (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (uint32_t *)a.out,
+                              a.n_streams, a.n, c);
+}
+
 }  // namespace
 
 cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
@@ -646,10 +982,20 @@ cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *
     // Kernel choice by stream count (measured on B200): 32 streams per CTA need >= ~128
     // CTAs; below that 8 streams per CTA; below ~1000 streams 4 per CTA in sector-sharing cluster pairs.
     int cfg = a.n_streams >= 4096 ? 0 : a.n_streams >= 1024 ? 1 : 2;
-    if (const char *env = std::getenv("PRAND_MT_CFG")) cfg = std::atoi(env);   // test hook: force a variant
+    // 4-byte outputs, 16-byte aligned rows: the cluster-gather kernel writes 64-byte pieces
+    const bool gather_ok = a.dtype != DT_F64 && a.n_streams % 4 == 0 && (uintptr_t)a.out % 16 == 0 && a.n / NW < (1ull << 32);
+    // (not the default: measured 1.29 ms on C3 against 1.00 ms for the cluster-pair kernel -- the exchange is
+    // bound by the ~10-13 B/clk/SM that distributed shared memory moves between four CTAs)
+    if (const char *env = std::getenv("PRAND_MT_CFG")) {                      // test hook: force a variant
+        const int want = std::atoi(env);
+        if (want != 3 || gather_ok) cfg = want;
+    }
     switch (cfg) {
     case 0: li->kernel = "mt19937_bgen<S=32>"; return dispatch_bdt<0>(stream, a);
     case 1: li->kernel = "mt19937_gen<S=8,T=104>"; return dispatch_dt<8, 104, 2, 0, false>(stream, a);
+    case 3:
+        li->kernel = "mt19937_cgen<CS=4>";
+        return a.dtype == DT_U32 ? launch_cgen<DT_U32>(stream, a) : launch_cgen<DT_F32>(stream, a);
     default: li->kernel = "mt19937_gen<S=4,T=208,pair>"; return dispatch_dt<4, 208, 1, 6, true>(stream, a);
     }
 }

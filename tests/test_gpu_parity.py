@@ -86,16 +86,25 @@ def test_every_output_and_state_matches_oracle(gen, dtype):
         assert st == wst, f"{w.name} {gen}: exported states differ"
 
 
-@pytest.mark.parametrize("cfg", range(3))
+MT_CFG_KERNEL = {0: "mt19937_bgen<S=32>", 1: "mt19937_gen<S=8,T=104>", 2: "mt19937_gen<S=4,T=208,pair>",
+                 3: "mt19937_cgen<CS=4>"}
+
+
+@pytest.mark.parametrize("cfg", range(4))
 def test_mt19937_every_kernel_configuration(cfg, monkeypatch):
-    """Every (streams per CTA, word slices, barrier interval, pipe mix, cluster pairing) variant of
-    the MT19937 generation kernel, over whole rounds of 624, several rounds and ragged tails, with
-    stream counts that leave CTAs partly or wholly dead."""
+    """Every (streams per CTA, word slices, barrier interval, pipe mix, cluster pairing / cluster
+    gather) variant of the MT19937 generation kernel, over whole rounds of 624, several rounds and
+    ragged tails, with stream counts that leave CTAs partly or wholly dead."""
     need_gpu()
     monkeypatch.setenv("PRAND_MT_CFG", str(cfg))
-    for ns, calls, dtype in [(5, [624, 1248, 1, 700], "u32"), (13, [2048], "f32"), (8, [1500, 623], "f64"), (70, [209, 1300], "u32")]:
+    cases = [(5, [624, 1248, 1, 700], "u32"), (13, [2048], "f32"), (8, [1500, 623], "f64"), (70, [209, 1300], "u32")]
+    if cfg == 3:      # the cluster-gather kernel takes 4-byte outputs and stream counts that are multiples of 4
+        cases = [(4, [624, 1248, 1, 700], "u32"), (12, [2048], "f32"), (16, [1500, 623, 3000], "u32"),
+                 (68, [209, 1300, 1872], "u32"), (36, [5000], "f32")]
+    for ns, calls, dtype in cases:
         w = Workload(f"mt-cfg{cfg}", "mt19937", 5489, ns, 1000, sum(calls), dtype)
-        got, st, _ = lib_run(w, calls=calls)
+        got, st, kernel = lib_run(w, calls=calls)
+        assert kernel == MT_CFG_KERNEL[cfg], kernel
         want, wst = oracle_run(w)
         assert_same(w, got, want)
         assert st == wst, f"cfg {cfg}: exported states differ"
