@@ -18,6 +18,7 @@ constexpr uint32_t C1 = 209u, C2 = 22853u;
 // small CTAs: with ~1000 CTAs on 148 SMs the most loaded SM is within 2% of the average
 constexpr int GEN_THREADS = 128;
 
+
 struct Mrg { uint32_t x0, x1, x2, y0, y1, y2; };   // x0 = x_n, x1 = x_{n-1}, x2 = x_{n-2}
 
 // x_{n+1} = (a x_{n-1} - b x_{n-2}) mod m1 from (x_{n-1}, x_{n-2}).  t = a x1 + b (m1 - x2) < 2^54,
@@ -234,11 +235,32 @@ __device__ __forceinline__ double mrg_next_yd(double y0, double y2)
     return __fma_rn(-k, 4294944443.0, p);
 }
 
+// Pipe-balanced forms for the 4-byte kernel, whose binding pipe is the ALU pipe (IADD3, ISETP, SHF, LOP3:
+// 64 lanes/clk/SM): additions whose operands allow it are written as multiply-adds with opaque register
+// multipliers (IMAD, FMA-heavy pipe); the multipliers are kernel arguments so that ptxas cannot turn them back
+// into ALU instructions.
+struct MrgK { uint32_t c1, neg1, m2; };
+__device__ __forceinline__ uint32_t mrg_next_x_b(uint32_t x1, uint32_t x2, const MrgK &k)
+{
+    const uint32_t nx2 = x2 * k.neg1 + M1;               // M1 - x2 as one IMAD
+    uint64_t t = (uint64_t)1403580u * x1 + (uint64_t)810728u * nx2;
+    uint32_t p = (uint32_t)(t >> 32) * k.c1 + k.c1;      // (hi + 1) * 209 < 2^30
+    uint32_t s = (uint32_t)t + p;
+    return s >= p ? s - C1 : s;                          // s >= p  <=>  no carry
+}
+__device__ __forceinline__ uint32_t mrg_y_out_b(double r, const MrgK &k)
+{
+    const uint32_t v = (uint32_t)__double2loint(__dadd_rn(r, 6755399441055744.0));
+    uint32_t y;                                          // + m2 for a negative representative: SHF + IMAD
+    asm("{.reg .u32 t; shr.u32 t, %1, 31; mad.lo.u32 %0, t, %2, %1;}" : "=r"(y) : "r"(v), "r"(k.m2));
+    return y;
+}
+
 template <int V, int DT>
 __global__ void __launch_bounds__(GEN_THREADS)
 mrg32k3a_gen_fp64y_kernel(const uint32_t *st_in, uint32_t *st_out,
                           typename OutElem<DT>::type *__restrict__ out, uint64_t ns, uint64_t n,
-                          uint64_t chunk_len, const MrgOp *__restrict__ chunk_ops)
+                          uint64_t chunk_len, const MrgOp *__restrict__ chunk_ops, const MrgK k)
 {
     typedef typename OutElem<DT>::type T;
     const uint64_t sg = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -258,32 +280,30 @@ mrg32k3a_gen_fp64y_kernel(const uint32_t *st_in, uint32_t *st_out,
     const uint64_t rows = (row0 + chunk_len < n) ? chunk_len : n - row0;
     T *p = out + row0 * ns + s0;
     T r[V];
-    uint32_t c1 = C1;
-    asm volatile("" : "+r"(c1));
     uint64_t i = 0;
 #pragma unroll 1
     for (; i + 3 <= rows; i += 3) {
 #pragma unroll
         for (int v = 0; v < V; v++) {
-            g[v].x2 = mrg_next_x(g[v].x1, g[v].x2, c1);
+            g[v].x2 = mrg_next_x_b(g[v].x1, g[v].x2, k);
             h[v].y2 = mrg_next_yd(h[v].y0, h[v].y2);
-            r[v] = mrg_output<DT>(g[v].x2, mrg_y_out(h[v].y2));
+            r[v] = mrg_output<DT>(g[v].x2, mrg_y_out_b(h[v].y2, k));
         }
         store_vec<V>(p, r);
         p += ns;
 #pragma unroll
         for (int v = 0; v < V; v++) {
-            g[v].x1 = mrg_next_x(g[v].x0, g[v].x1, c1);
+            g[v].x1 = mrg_next_x_b(g[v].x0, g[v].x1, k);
             h[v].y1 = mrg_next_yd(h[v].y2, h[v].y1);
-            r[v] = mrg_output<DT>(g[v].x1, mrg_y_out(h[v].y1));
+            r[v] = mrg_output<DT>(g[v].x1, mrg_y_out_b(h[v].y1, k));
         }
         store_vec<V>(p, r);
         p += ns;
 #pragma unroll
         for (int v = 0; v < V; v++) {
-            g[v].x0 = mrg_next_x(g[v].x2, g[v].x0, c1);
+            g[v].x0 = mrg_next_x_b(g[v].x2, g[v].x0, k);
             h[v].y0 = mrg_next_yd(h[v].y1, h[v].y0);
-            r[v] = mrg_output<DT>(g[v].x0, mrg_y_out(h[v].y0));
+            r[v] = mrg_output<DT>(g[v].x0, mrg_y_out_b(h[v].y0, k));
         }
         store_vec<V>(p, r);
         p += ns;
@@ -292,11 +312,11 @@ mrg32k3a_gen_fp64y_kernel(const uint32_t *st_in, uint32_t *st_out,
     for (; i < rows; i++) {                              // ragged tail: rotate by moving
 #pragma unroll
         for (int v = 0; v < V; v++) {
-            const uint32_t nx = mrg_next_x(g[v].x1, g[v].x2, c1);
+            const uint32_t nx = mrg_next_x_b(g[v].x1, g[v].x2, k);
             const double ny = mrg_next_yd(h[v].y0, h[v].y2);
             g[v].x2 = g[v].x1; g[v].x1 = g[v].x0; g[v].x0 = nx;
             h[v].y2 = h[v].y1; h[v].y1 = h[v].y0; h[v].y0 = ny;
-            r[v] = mrg_output<DT>(nx, mrg_y_out(ny));
+            r[v] = mrg_output<DT>(nx, mrg_y_out_b(ny, k));
         }
         store_vec<V>(p, r);
         p += ns;
@@ -375,7 +395,7 @@ template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenAr
     if (DT != DT_F64 && !int_only)
         mrg32k3a_gen_fp64y_kernel<V, DT><<<grid, GEN_THREADS, 0, stream>>>(
             (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
-            (const MrgOp *)a.chunk_ops);
+            (const MrgOp *)a.chunk_ops, MrgK{C1, 0xFFFFFFFFu, M2});
     else
         mrg32k3a_gen_kernel<V, DT><<<grid, GEN_THREADS, 0, stream>>>(
             (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,
