@@ -68,9 +68,10 @@ cudaError_t lfsr113_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
 cudaError_t lfsr113_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
 cudaError_t mrg32k3a_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
 cudaError_t mrg32k3a_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
-// sections of one sequence written in PRAND's contiguous layout (sec_len a multiple of 16, out 16-byte aligned)
-cudaError_t mrg32k3a_seq_f64(cudaStream_t, const void *st_in, double *out, uint64_t n_sections, uint64_t sec_len,
-                             uint64_t length, LaunchInfo *);
+// sections of one sequence written in PRAND's contiguous layout (sec_len a multiple of 16, out 16-byte aligned);
+// st_last (one stream) receives the state of the sequence after `length` numbers
+cudaError_t mrg32k3a_seq_f64(cudaStream_t, const void *st_in, void *st_last, double *out, uint64_t n_sections,
+                             uint64_t sec_len, uint64_t length, LaunchInfo *);
 cudaError_t gm_jump(cudaStream_t, int gen, const JumpArgs &, LaunchInfo *);
 cudaError_t gm_generate(cudaStream_t, int gen, const GenArgs &, LaunchInfo *);
 // streams [s_begin, s_end) = kn * stream(s - back) - qn * stream(s - 2 back) (eq. 2), in place
@@ -81,6 +82,10 @@ cudaError_t gm_tree_fill(cudaStream_t, int gen, void *st, uint64_t ns, uint64_t 
 cudaError_t mt19937_apply(cudaStream_t, const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
                           uint64_t count, uint64_t src_back, const MtOp *d_op, LaunchInfo *);
 cudaError_t mt19937_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
+// sections of one sequence in PRAND's contiguous layout out[c * sec_len + i] (sec_len even, out 16-byte aligned);
+// st_in = [n_sections][624] windows, st_last (one window) receives the state after `length` numbers
+cudaError_t mt19937_seq(cudaStream_t, const void *st_in, void *st_last, void *out, int dtype, uint64_t n_sections,
+                        uint64_t sec_len, uint64_t length, LaunchInfo *);
 cudaError_t fill_u32(cudaStream_t, uint32_t *out, uint64_t n_words, uint32_t value, LaunchInfo *);
 // out[c * sec_len + i] = tmp[i * n_sections + c] for c * sec_len + i < length (elem_bytes 4 or 8)
 cudaError_t transpose_sections(cudaStream_t, const void *tmp, void *out, uint64_t n_sections, uint64_t sec_len,

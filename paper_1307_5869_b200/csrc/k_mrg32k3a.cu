@@ -331,46 +331,57 @@ mrg32k3a_gen_fp64y_kernel(const uint32_t *st_in, uint32_t *st_out,
 }
 
 // ---- sections of a single sequence, float64 (prand_generate_seq_f64; the paper's Table 7 task) -------
-// Thread t owns sections 2t and 2t+1 (as in the bulk kernel) but the array layout is PRAND's
-// contiguous one, out[c * sec_len + i].  A warp collects 16 rows of its 64 sections in a
-// shared-memory tile and writes them section by section: eight lanes store the 128 contiguous bytes of
-// one section's 16 numbers, so a warp store covers four full 128-byte lines.
+// The array layout is PRAND's contiguous one, out[c * sec_len + i].  A warp owns 32 V
+// consecutive sections, lane k the sections k, k + 32, ...  It collects 16 rows of its sections in a
+// shared-memory tile (pitch 17 doubles: a lane's stores hit 16 different bank pairs, conflict-free) and
+// writes them section by section: eight lanes store the 128 contiguous bytes of one section's 16 numbers,
+// so a warp store covers four full lines.  V = 1 with up to 2^17 sections fills the GPU with one wave of
+// 28 warps per SM; V = 2 serves fewer, longer sections.  The last section's state after its last row is
+// the state of the whole sequence after `length` numbers: it goes to st_last, no final jump is needed.
 constexpr int SEQ_ROWS = 16, SEQ_PITCH = 17;               // tile[section][row], pitch in doubles
 
-__global__ void __launch_bounds__(GEN_THREADS)
-mrg32k3a_seq_f64_kernel(const uint32_t *st_in, double *__restrict__ out, uint64_t n_sections, uint64_t sec_len,
-                        uint64_t length)
+template <int V>
+__global__ void __launch_bounds__(GEN_THREADS, V == 1 ? 7 : 1)
+mrg32k3a_seq_f64_kernel(const uint32_t *st_in, uint32_t *st_last, double *__restrict__ out, uint64_t n_sections,
+                        uint64_t sec_len, uint64_t length)
 {
-    __shared__ double tile_all[GEN_THREADS / 32][64 * SEQ_PITCH];
+    __shared__ double tile_all[GEN_THREADS / 32][32 * V * SEQ_PITCH];
     double *tile = tile_all[threadIdx.x >> 5];
     const int lane = threadIdx.x & 31;
-    const uint64_t warp_sec0 = ((uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u)) * 2;   // first section of the warp
+    const uint64_t warp_sec0 = ((uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u)) * V;   // first section of the warp
     if (warp_sec0 >= n_sections) return;                   // whole warp
-    const uint64_t s0 = warp_sec0 + 2 * lane;
-    Mrg g[2];
+    Mrg g[V];
 #pragma unroll
-    for (int v = 0; v < 2; v++) g[v] = mrg_load(st_in, n_sections, s0 + v < n_sections ? s0 + v : n_sections - 1);
+    for (int v = 0; v < V; v++) {
+        const uint64_t sec = warp_sec0 + 32 * v + lane;
+        g[v] = mrg_load(st_in, n_sections, sec < n_sections ? sec : n_sections - 1);
+    }
     uint32_t c1 = C1;
     asm volatile("" : "+r"(c1));
     // rows of the warp's sections: sec_len for all but the last section of the array
     const uint64_t last = n_sections - 1;
     const uint64_t last_rows = length - last * sec_len;
+    const bool has_last = warp_sec0 + 32 * V > last;       // this warp owns the last section ...
+    const int last_v = has_last ? (int)((last - warp_sec0) >> 5) : 0;   // ... as recurrence last_v of lane (last - warp_sec0) % 32
+    const bool owns_last = has_last && lane == (int)((last - warp_sec0) & 31);
 #pragma unroll 1
     for (uint64_t i0 = 0; i0 < sec_len; i0 += SEQ_ROWS) {
+        const int snap = owns_last && last_rows >= i0 && last_rows < i0 + SEQ_ROWS ? (int)(last_rows - i0) : -1;
 #pragma unroll
         for (int r = 0; r < SEQ_ROWS; r++) {
+            if (r == snap) mrg_store(st_last, 1, 0, g[last_v]);
 #pragma unroll
-            for (int v = 0; v < 2; v++) {
+            for (int v = 0; v < V; v++) {
                 const uint32_t nx = mrg_next_x(g[v].x1, g[v].x2, c1), ny = mrg_next_y(g[v].y0, g[v].y2);
                 g[v].x2 = g[v].x1; g[v].x1 = g[v].x0; g[v].x0 = nx;
                 g[v].y2 = g[v].y1; g[v].y1 = g[v].y0; g[v].y0 = ny;
-                tile[(2 * lane + v) * SEQ_PITCH + r] = mrg_output<DT_F64>(nx, ny);
+                tile[(32 * v + lane) * SEQ_PITCH + r] = mrg_output<DT_F64>(nx, ny);
             }
         }
         __syncwarp();
         const int sub = lane >> 3, piece = lane & 7;
 #pragma unroll 4
-        for (int k = 0; k < 16; k++) {
+        for (int k = 0; k < 8 * V; k++) {
             const int sl = 4 * k + sub;                    // section within the warp
             const uint64_t sec = warp_sec0 + sl;
             const uint64_t row = i0 + 2 * piece;
@@ -384,6 +395,7 @@ mrg32k3a_seq_f64_kernel(const uint32_t *st_in, double *__restrict__ out, uint64_
         }
         __syncwarp();
     }
+    if (owns_last && last_rows == sec_len) mrg_store(st_last, 1, 0, g[last_v]);
 }
 
 template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
@@ -426,12 +438,19 @@ cudaError_t mrg32k3a_jump(cudaStream_t stream, const JumpArgs &a, LaunchInfo *li
     return cudaGetLastError();
 }
 
-cudaError_t mrg32k3a_seq_f64(cudaStream_t stream, const void *st_in, double *out, uint64_t n_sections,
+cudaError_t mrg32k3a_seq_f64(cudaStream_t stream, const void *st_in, void *st_last, double *out, uint64_t n_sections,
                              uint64_t sec_len, uint64_t length, LaunchInfo *li)
 {
-    const uint64_t threads = ceil_div_u64(n_sections, 2);
-    mrg32k3a_seq_f64_kernel<<<(unsigned)ceil_div_u64(threads, GEN_THREADS), GEN_THREADS, 0, stream>>>(
-        (const uint32_t *)st_in, out, n_sections, sec_len, length);
+    // one section per thread when there are enough of them to fill the GPU, else two (more work in flight per thread)
+    if (n_sections >= 32768) {
+        const uint64_t threads = ceil_div_u64(n_sections, 32) * 32;
+        mrg32k3a_seq_f64_kernel<1><<<(unsigned)ceil_div_u64(threads, GEN_THREADS), GEN_THREADS, 0, stream>>>(
+            (const uint32_t *)st_in, (uint32_t *)st_last, out, n_sections, sec_len, length);
+    } else {
+        const uint64_t threads = ceil_div_u64(n_sections, 64) * 32;
+        mrg32k3a_seq_f64_kernel<2><<<(unsigned)ceil_div_u64(threads, GEN_THREADS), GEN_THREADS, 0, stream>>>(
+            (const uint32_t *)st_in, (uint32_t *)st_last, out, n_sections, sec_len, length);
+    }
     li->kernel = "mrg32k3a_seq_f64";
     li->launches = 1;
     return cudaGetLastError();

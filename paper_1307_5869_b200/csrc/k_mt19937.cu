@@ -681,7 +681,13 @@ __device__ __forceinline__ void cluster_sync_all()
 }
 __device__ __forceinline__ void group_barrier(int g)
 {
-    asm volatile("bar.sync %0, %1;" :: "r"(1 + g), "n"(CG_GT) : "memory");
+    // compile-time barrier numbers: a register operand would reserve all 16 hardware barriers for the CTA
+    switch (g) {
+    case 0: asm volatile("bar.sync 1, %0;" :: "n"(CG_GT) : "memory"); break;
+    case 1: asm volatile("bar.sync 2, %0;" :: "n"(CG_GT) : "memory"); break;
+    case 2: asm volatile("bar.sync 3, %0;" :: "n"(CG_GT) : "memory"); break;
+    default: asm volatile("bar.sync 4, %0;" :: "n"(CG_GT) : "memory"); break;
+    }
 }
 template <int DT> __device__ __forceinline__ uint32_t out_bits(uint32_t u)
 {
@@ -705,6 +711,21 @@ __device__ __forceinline__ void cg_operands(const uint32_t *smem, const uint32_t
         m0 = smem[q]; m1 = smem[q + 1];
     }
 }
+// The two recurrences of a wave from their operands; (p0, p1) receive the new words.
+template <int J>
+__device__ __forceinline__ void cg_step(uint32_t *smem, const uint32_t ia, const uint32_t ib, const int u, uint32_t (&r)[6],
+                                        const MtMul &c, const uint32_t x2, const uint32_t m0, const uint32_t m1,
+                                        uint32_t &p0, uint32_t &p1)
+{
+    const uint32_t n0 = mt_recur2<0>(r[2 * J], r[2 * J + 1], m0, c);
+    const uint32_t n1 = mt_recur2<0>(r[2 * J + 1], x2, m1, c);
+    r[2 * J] = n0;
+    r[2 * J + 1] = n1;
+    *reinterpret_cast<uint2 *>(smem + ib + CG_T * J) = make_uint2(n0, n1);
+    if (J == 0 && u == 0) smem[ia + NW] = n0;
+    p0 = n0;
+    p1 = n1;
+}
 // Full wave.  (p0, p1) carry the previous wave's two new words, whose tempering and staging store (slot
 // pend_slot of tile sb) run here, after this wave's loads have been issued, if `pending`.
 template <int J, int DT>
@@ -716,14 +737,7 @@ __device__ __forceinline__ void cg_wave(uint32_t *smem, const uint32_t ia, const
     cg_operands<J>(smem, ia, ib, u, x2, m0, m1);
     if (pending)
         *reinterpret_cast<uint2 *>(sb + pend_slot) = make_uint2(out_bits<DT>(mt_temper2<0>(p0, c)), out_bits<DT>(mt_temper2<0>(p1, c)));
-    const uint32_t n0 = mt_recur2<0>(r[2 * J], r[2 * J + 1], m0, c);
-    const uint32_t n1 = mt_recur2<0>(r[2 * J + 1], x2, m1, c);
-    r[2 * J] = n0;
-    r[2 * J + 1] = n1;
-    *reinterpret_cast<uint2 *>(smem + ib + CG_T * J) = make_uint2(n0, n1);
-    if (J == 0 && u == 0) smem[ia + NW] = n0;
-    p0 = n0;
-    p1 = n1;
+    cg_step<J>(smem, ia, ib, u, r, c, x2, m0, m1, p0, p1);
 }
 // Ragged tail: only words below `rem` are produced; (o0, o1) = the converted outputs.
 template <int J, int DT>
@@ -914,6 +928,120 @@ mt19937_cgen_kernel(const uint32_t *st_in, uint32_t *st_out, uint32_t *__restric
     }
 }
 
+// ---- sections of a single sequence (prand_generate_seq_*; Table 5) ----------------------
+// Section c = stream c of the family, its numbers contiguous in memory: out[c * sec_len + i].  With the
+// per-stream thread groups of the kernel above (thread = two adjacent words of a wave, 104 threads per
+// stream) a warp's store is 64 consecutive rows of ONE section: 256 (u32, f32) or 512 (f64) contiguous
+// bytes straight from registers -- no exchange, no staging, no transposition.  Four sections per CTA,
+// each group running at its own pace (named barriers); the last section of the array may be shorter
+// and its final window, the state of the sequence after `length` numbers, goes to st_last.
+template <int DT> __device__ __forceinline__ void sg_store2(typename OutElem<DT>::type *p, uint32_t a, uint32_t b)
+{
+    store2(p, convert<DT>(a), convert<DT>(b));
+}
+
+template <int DT>
+__global__ void __launch_bounds__(CG_CT, 2)
+mt19937_sgen_kernel(const uint32_t *st_in, uint32_t *st_last, typename OutElem<DT>::type *__restrict__ out,
+                    uint64_t n_sections, uint64_t sec_len, uint64_t length, const MtMul c)
+{
+    typedef typename OutElem<DT>::type E;
+    extern __shared__ __align__(16) uint32_t smem[];     // windows [2][S][P]
+    const int tid = threadIdx.x;
+    const int g = tid / CG_GT, tg = tid % CG_GT;
+    const uint64_t sec0 = (uint64_t)blockIdx.x * CG_S, sec = sec0 + g;
+    const bool live = sec < n_sections;
+    const bool act = live && tg < CG_U;
+    const int u = act ? tg : 0;
+    const int n_live = sec0 >= n_sections ? 0 : (n_sections - sec0 < (uint64_t)CG_S ? (int)(n_sections - sec0) : CG_S);
+    for (int i = tid; i < CG_S * (NW / 4); i += CG_CT) {
+        const int q = i / (NW / 4), w4 = i % (NW / 4);
+        if (q < n_live) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4 *>(st_in + (sec0 + q) * NW) + w4);
+            *reinterpret_cast<uint4 *>(smem + q * CG_P + 4 * w4) = v;
+        }
+    }
+    __syncthreads();
+    const uint64_t last = n_sections - 1;
+    const uint64_t rows = !live ? 0 : (sec == last ? length - last * sec_len : sec_len);
+    const uint32_t rounds = (uint32_t)(rows / NW);
+    const int rem = (int)(rows % NW);
+    uint32_t ia = g * CG_P + 2 * u, ib = ia + CG_S * CG_P;
+    uint32_t r[6] = {0u, 0u, 0u, 0u, 0u, 0u};
+    if (act) {
+#pragma unroll
+        for (int j = 0; j < 3; j++) { r[2 * j] = smem[ia + CG_T * j]; r[2 * j + 1] = smem[ia + CG_T * j + 1]; }
+    }
+    E *p = out + sec * sec_len + 2 * u;
+    // as in the cluster kernel the tempering and the store of a wave's two numbers are deferred until the next
+    // wave's shared loads have been issued (they fill the wait after the barrier)
+    uint32_t p0 = 0, p1 = 0;
+    for (uint32_t rd = 0; rd < rounds; rd++, p += NW) {
+        if (act) {
+            uint32_t x2, m0, m1;
+            cg_operands<0>(smem, ia, ib, u, x2, m0, m1);
+            if (rd) sg_store2<DT>(p - NW + 2 * CG_T, mt_temper2<0>(p0, c), mt_temper2<0>(p1, c));
+            cg_step<0>(smem, ia, ib, u, r, c, x2, m0, m1, p0, p1);
+        }
+        group_barrier(g);
+        if (act) {
+            uint32_t x2, m0, m1;
+            cg_operands<1>(smem, ia, ib, u, x2, m0, m1);
+            sg_store2<DT>(p, mt_temper2<0>(p0, c), mt_temper2<0>(p1, c));
+            cg_step<1>(smem, ia, ib, u, r, c, x2, m0, m1, p0, p1);
+        }
+        group_barrier(g);
+        if (act) {
+            uint32_t x2, m0, m1;
+            cg_operands<2>(smem, ia, ib, u, x2, m0, m1);
+            sg_store2<DT>(p + CG_T, mt_temper2<0>(p0, c), mt_temper2<0>(p1, c));
+            cg_step<2>(smem, ia, ib, u, r, c, x2, m0, m1, p0, p1);
+        }
+        group_barrier(g);
+        { const uint32_t tmp = ia; ia = ib; ib = tmp; }
+    }
+    if (act && rounds) sg_store2<DT>(p - NW + 2 * CG_T, mt_temper2<0>(p0, c), mt_temper2<0>(p1, c));
+    if (rem) {                                             // only the last section of the array is ragged
+        uint32_t o0 = 0, o1 = 0;
+#define PRAND_SG_TAIL(J)                                                                      \
+        if (act) {                                                                            \
+            const int w = CG_T * J + 2 * u;                                                   \
+            cg_tail_wave<J, DT_U32>(smem, ia, ib, u, r, c, o0, o1, rem);                      \
+            if (w < rem) store1(p + CG_T * J, convert<DT>(o0));                               \
+            if (w + 1 < rem) store1(p + CG_T * J + 1, convert<DT>(o1));                       \
+        }                                                                                     \
+        group_barrier(g);
+        PRAND_SG_TAIL(0)
+        PRAND_SG_TAIL(1)
+        PRAND_SG_TAIL(2)
+#undef PRAND_SG_TAIL
+    }
+    // the sequence after `length` numbers: final window of the last section = words [rem, 624) of its old
+    // buffer, then [0, rem) of the new one (written by that section's own group)
+    if (live && sec == last) {
+        const uint32_t cur = rounds & 1;
+        const uint32_t *a0 = smem + cur * (CG_S * CG_P) + g * CG_P, *b0 = smem + (cur ^ 1) * (CG_S * CG_P) + g * CG_P;
+        for (int j = tg; j < NW; j += CG_GT) {
+            const int pp = j + rem;
+            st_last[j] = pp < NW ? a0[pp] : b0[pp - NW];
+        }
+    }
+}
+
+template <int DT> cudaError_t launch_sgen(cudaStream_t stream, const void *st_in, void *st_last, void *out,
+                                          uint64_t n_sections, uint64_t sec_len, uint64_t length)
+{
+    typedef typename OutElem<DT>::type E;
+    auto kern = mt19937_sgen_kernel<DT>;
+    const size_t smem = (size_t)2 * CG_S * CG_P * sizeof(uint32_t);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const MtMul c = {2u * 0x1908B0DFu, 1u << 31, 1u << 21, 1u << 14};
+    kern<<<(unsigned)ceil_div_u64(n_sections, CG_S), CG_CT, smem, stream>>>((const uint32_t *)st_in, (uint32_t *)st_last,
+                                                                           (E *)out, n_sections, sec_len, length, c);
+    return cudaGetLastError();
+}
+
 template <int DT> cudaError_t launch_cgen(cudaStream_t stream, const GenArgs &a)
 {
     auto kern = mt19937_cgen_kernel<DT>;
@@ -972,6 +1100,18 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
         mt19937_apply_win_kernel<<<(unsigned)count, APPLYW_THREADS, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     li->launches = 1;
     return cudaGetLastError();
+}
+
+cudaError_t mt19937_seq(cudaStream_t stream, const void *st_in, void *st_last, void *out, int dtype, uint64_t n_sections,
+                        uint64_t sec_len, uint64_t length, LaunchInfo *li)
+{
+    li->kernel = "mt19937_sgen<S=4>";
+    li->launches = 1;
+    switch (dtype) {
+    case DT_U32: return launch_sgen<DT_U32>(stream, st_in, st_last, out, n_sections, sec_len, length);
+    case DT_F32: return launch_sgen<DT_F32>(stream, st_in, st_last, out, n_sections, sec_len, length);
+    default: return launch_sgen<DT_F64>(stream, st_in, st_last, out, n_sections, sec_len, length);
+    }
 }
 
 cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *li)

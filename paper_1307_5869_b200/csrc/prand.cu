@@ -675,11 +675,12 @@ namespace {
 // reached by jump-ahead and filled in parallel; the result is what the serial generator would have
 // produced.  Here: section c = a stream that starts c * sec_len ahead of the state, the family is
 // filled in the interleaved layout by the bulk kernels and transposed into out[c * sec_len + i].
-void plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec_len)
+void plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec_len, int sms = 148)
 {
     // enough sections to fill the GPU, sections long enough to amortise the jump to their start
     const uint64_t min_len = gen == PRAND_MT19937 ? 8 * 624 : 1024;
-    const uint64_t max_sec = gen == PRAND_MT19937 ? 1024 : 65536;   // MT19937: one 0.2 ms jump level per doubling
+    // MT19937: every section costs a polynomial application (~1 us of a whole SM): one CTA of four sections per SM
+    const uint64_t max_sec = gen == PRAND_MT19937 ? 4 * (uint64_t)sms : 131072;
     uint64_t S = length / min_len;
     if (S > max_sec) S = max_sec;
     if (S < 1) S = 1;
@@ -695,7 +696,7 @@ int generate_seq(prand_state *st, void *out, uint64_t length, int dtype, cudaStr
     if (st->ns != 1) return PRAND_ERR_ARG;                 // one sequence: the state of a single stream
     if (length == 0) return PRAND_OK;
     uint64_t S, L;
-    plan_sections(st->gen, length, &S, &L);
+    plan_sections(st->gen, length, &S, &L, sm_count());
     if (S == 1) return generate(st, out, length, dtype, stream);
     st->last_stream = stream;
     const size_t esz = dtype == DT_F64 ? 8 : 4;
@@ -726,9 +727,16 @@ int generate_seq(prand_state *st, void *out, uint64_t length, int dtype, cudaStr
     if (st->gen == PRAND_MRG32K3A && dtype == DT_F64 && (uintptr_t)out % 16 == 0) {
         // fused path: the sections are written in place, no scratch buffer, no transposition
         LaunchInfo li;
-        CU(mrg32k3a_seq_f64(stream, c->d_state[c->cur], (double *)out, S, L, length, &li));
+        CU(mrg32k3a_seq_f64(stream, c->d_state[c->cur], st->d_state[st->cur], (double *)out, S, L, length, &li));
         note(st, li);
-        return prand_jump(st, length, 0, stream);
+        return PRAND_OK;                                       // the kernel left the advanced state in st
+    }
+    if (st->gen == PRAND_MT19937 && (uintptr_t)out % 16 == 0) {
+        // per-stream thread groups write each section's numbers as contiguous runs straight from registers
+        LaunchInfo li;
+        CU(mt19937_seq(stream, c->d_state[c->cur], st->d_state[st->cur], out, dtype, S, L, length, &li));
+        note(st, li);
+        return PRAND_OK;
     }
     void *tmp = nullptr;
     CU(dev_alloc(&tmp, (size_t)L * S * esz, stream));
