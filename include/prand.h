@@ -158,10 +158,37 @@ int prand_generate_strided_f64(prand_state *st, double *out, uint64_t n_per_stre
  * include/prand_device.cuh holds the header-only __device__ generators; these calls give a kernel
  * access to the library's device-resident state (layout documented in that header; the pointer stays
  * valid until the next prand_generate_* call that uses sub-sections, prand_set_state or prand_free)
- * and run the library's own example kernel written against that header: one thread per stream,
+ * and run the library's own example kernel written against that header: one thread per stream (MT19937:
+ * one warp per stream on a shared-memory window),
  * out[i * n_streams + s] as for prand_generate_*, the streams advance by n_per_stream.  The example
  * is a self-test of the header, not a fast path.
  */
+/*
+ * prand_device_ops -- operator table for skip-ahead INSIDE a user's kernel (PRAND's
+ *   `*_init_device_consts_` places the tables that `*_dev_skipahead_` / `*_dev_init_sequence_` use in
+ *   device memory).  Builds the skip operators of generator prand_gen_of(st) for the distances
+ *   dist * 2^j, j = 0 .. levels-1 (dist = dist_mant * 2^dist_log2), uploads them and returns in *d_ops a
+ *   DEVICE pointer to an array of `levels` operators (prand_lfsr113_op / prand_mrg32k3a_op /
+ *   prand_mt19937_op / prand_gm_op of include/prand_ops.h): prand_dev::Gen<GEN>::skipahead(ops, s)
+ *   advances a stream by s * dist for any s < 2^levels.  The table is owned by `st` and stays valid until
+ *   the next prand_device_ops call on `st` or prand_free.  1 <= levels <= 64.  Synchronises the stream.
+ *
+ * prand_device_api_init_fill_{u32,f32,f64} -- the library's example kernel for that path: `st` holds ONE
+ *   stream (the base stream, else PRAND_ERR_ARG); every stream s < n_streams is initialised on the device
+ *   (base stream loaded, skipped s * block_len ahead with the table) and generates n_per_stream numbers
+ *   into out[i * n_streams + s] -- exactly the numbers of prand_init(..., n_streams, block_len) +
+ *   prand_generate_*.  MT19937 runs one CTA per stream (CTA-cooperative skip, warp-cooperative generator).
+ *   The base state is not modified.
+ */
+int prand_device_ops(prand_state *st, uint64_t dist_mant, unsigned dist_log2, unsigned levels,
+                     const void **d_ops, void *cuda_stream);
+int prand_device_api_init_fill_u32(prand_state *st, uint64_t block_len_mant, unsigned block_len_log2,
+                                   uint64_t n_streams, uint32_t *out, uint64_t n_per_stream, void *cuda_stream);
+int prand_device_api_init_fill_f32(prand_state *st, uint64_t block_len_mant, unsigned block_len_log2,
+                                   uint64_t n_streams, float *out, uint64_t n_per_stream, void *cuda_stream);
+int prand_device_api_init_fill_f64(prand_state *st, uint64_t block_len_mant, unsigned block_len_log2,
+                                   uint64_t n_streams, double *out, uint64_t n_per_stream, void *cuda_stream);
+
 void *prand_state_device_ptr(prand_state *st);
 uint64_t prand_state_n_streams(const prand_state *st);
 int prand_device_api_fill_u32(prand_state *st, uint32_t *out, uint64_t n_per_stream, void *cuda_stream);

@@ -7,8 +7,49 @@
 #pragma once
 #include <stdint.h>
 #include "prand.h"
+#include "prand_ops.h"
 
 namespace prand_dev {
+
+/* ---- skip-ahead: 2x2 companion-matrix powers mod g, Barrett reduction ----------
+ * g < 2^61; mu = floor(2^(2 nb) / g) with nb = bit length of g. */
+struct Barrett { uint64_t g, mu; unsigned nb; };
+
+__host__ __device__ constexpr unsigned gm_bit_length(uint64_t x) { return x ? 1u + gm_bit_length(x >> 1) : 0u; }
+__host__ __device__ constexpr Barrett gm_barrett(uint64_t g)
+{
+    return Barrett{g, (uint64_t)((((unsigned __int128)1) << (2 * gm_bit_length(g))) / g), gm_bit_length(g)};
+}
+__device__ __forceinline__ uint64_t bmulmod(uint64_t a, uint64_t b, const Barrett &B)
+{
+    uint64_t lo = a * b, hi = __umul64hi(a, b);                      // x = a b < g^2 < 2^(2 nb)
+    uint64_t q1 = (hi << (65 - B.nb)) | (lo >> (B.nb - 1));          // x >> (nb-1) < 2^(nb+1)
+    uint64_t l2 = q1 * B.mu, h2 = __umul64hi(q1, B.mu);
+    uint64_t q3 = (h2 << (63 - B.nb)) | (l2 >> (B.nb + 1));          // floor(q1 mu / 2^(nb+1))
+    uint64_t r = lo - q3 * B.g;                                      // 0 <= x - q3 g < 3 g < 2^64
+    while (r >= B.g) r -= B.g;
+    return r;
+}
+__device__ __forceinline__ uint64_t baddmod(uint64_t a, uint64_t b, const Barrett &B)
+{
+    uint64_t t = a + b;                                              // < 2^62
+    return t >= B.g ? t - B.g : t;
+}
+// (xN, xP) <- product of ops[b] over the set bits b of idx, applied to the column (x(n), x(n-1)).
+// noinline: callers invoke it once per register-resident point (static indexing keeps the ensemble
+// out of local memory) and it is cold
+static __device__ __noinline__ void gm_apply_bits(const prand_gm_op *__restrict__ ops, uint64_t idx, uint64_t &xP,
+                                           uint64_t &xN, const Barrett &B)
+{
+    for (int lev = 0; idx != 0; lev++, idx >>= 1)
+        if (idx & 1) {
+            uint64_t m0 = __ldg(&ops[lev].m[0]), m1 = __ldg(&ops[lev].m[1]);
+            uint64_t m2 = __ldg(&ops[lev].m[2]), m3 = __ldg(&ops[lev].m[3]);
+            uint64_t n = baddmod(bmulmod(m0, xN, B), bmulmod(m1, xP, B), B);
+            uint64_t o = baddmod(bmulmod(m2, xN, B), bmulmod(m3, xP, B), B);
+            xN = n; xP = o;
+        }
+}
 
 // Traits of one generator.  W = canonical state word in HBM (a residue mod g), R = the word the
 // generation loop keeps in registers, load/store convert between them at the ends of a call.
@@ -36,6 +77,7 @@ template <> struct Gm<PRAND_GM19> {
     static constexpr int S = 32;
     static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint32_t G = (1u << 19) - 1;
+    static constexpr uint64_t MODULUS = G;
     __device__ static __forceinline__ R load(W x) { return x; }
     __device__ static __forceinline__ W store(R x) { return x; }
     __device__ static __forceinline__ R step(R xP, R xN)
@@ -56,6 +98,7 @@ template <> struct Gm<PRAND_GM29> {
     static constexpr int S = 32;
     static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint32_t G = (1u << 29) - 3;
+    static constexpr uint64_t MODULUS = G;
     __device__ static __forceinline__ R load(W x) { return x; }
     __device__ static __forceinline__ W store(R x) { return x; }
     __device__ static __forceinline__ R step(R xP, R xN)
@@ -80,6 +123,7 @@ template <> struct Gm<PRAND_GM31> {
     static constexpr int S = 32;
     static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint32_t G = (1u << 31) - 1;
+    static constexpr uint64_t MODULUS = G;
     __device__ static __forceinline__ R load(W x) { return x; }
     __device__ static __forceinline__ W store(R x) { return x; }
     __device__ static __forceinline__ R step(R xP, R xN)
@@ -108,6 +152,7 @@ template <> struct Gm<PRAND_GM61> {
     typedef uint64_t R;
     static constexpr int S = 32;
     static constexpr bool PACK_DESCENDING = true, NEEDS_CLEAN = false, HAS_FAST = true;
+    static constexpr uint64_t MODULUS = (1ull << 61) - 1;
     __device__ static __forceinline__ R load(W x) { return x << 3; }
     __device__ static __forceinline__ W store(R x) { return x >> 3; }
     __device__ static __forceinline__ R step(R XP, R XN)
@@ -293,6 +338,7 @@ template <> struct GmPlain<PRAND_GM55> {
     static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint64_t P = (1ull << 51) - 129;
     static constexpr uint64_t G = 16ull * P;
+    static constexpr uint64_t MODULUS = G;
     __device__ static __forceinline__ R load(W x) { return x; }
     __device__ static __forceinline__ W store(R x) { return x; }
     __device__ static __forceinline__ R step(R xP, R xN)
@@ -318,6 +364,7 @@ template <int VB, int SS> struct Gq58Plain {
     static constexpr bool PACK_DESCENDING = false, NEEDS_CLEAN = false, HAS_FAST = false;
     static constexpr uint64_t P = (1ull << 29) - 3;
     static constexpr uint64_t G = P << 29;
+    static constexpr uint64_t MODULUS = G;
     __device__ static __forceinline__ R load(W x) { return x; }
     __device__ static __forceinline__ W store(R x) { return x; }
     __device__ static __forceinline__ R step(R xP, R xN)
@@ -368,6 +415,18 @@ template <class Tr> struct GmGen {
         for (int i = 0; i < Tr::S; i++) {
             b[(uint64_t)(2 * i) * ns + s] = Tr::store(xP[i]);
             b[(uint64_t)(2 * i + 1) * ns + s] = Tr::store(xN[i]);
+        }
+    }
+    /* every ensemble point advanced by idx * dist (ops from prand_device_ops(dist, levels)) */
+    __device__ void skipahead(const prand_gm_op *ops, uint64_t idx)
+    {
+        const Barrett B = gm_barrett(Tr::MODULUS);
+#pragma unroll
+        for (int i = 0; i < Tr::S; i++) {
+            uint64_t a = Tr::store(xP[i]), b = Tr::store(xN[i]);
+            gm_apply_bits(ops, idx, a, b, B);
+            xP[i] = Tr::load((W)a);
+            xN[i] = Tr::load((W)b);
         }
     }
     __device__ uint32_t next_u32()

@@ -45,6 +45,10 @@ _SIGS = {
     "prand_device_api_fill_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_device_api_fill_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_device_api_fill_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_device_ops": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint, C.c_uint, C.POINTER(C.c_void_p), C.c_void_p]),
+    "prand_device_api_init_fill_u32": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_device_api_init_fill_f32": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_device_api_init_fill_f64": (C.c_int, [C.c_void_p, C.c_uint64, C.c_uint, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_generate_strided_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint, C.c_void_p]),
     "prand_generate_strided_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint, C.c_void_p]),
     "prand_generate_strided_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint, C.c_void_p]),
@@ -298,6 +302,18 @@ class Generator:
         tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
         out = torch.empty((n_per_stream, self.n_streams), dtype=tdt, device="cuda")
         _generate("prand_device_api_fill_" + dtype, self._h, out.data_ptr(), n_per_stream, stream)
+        return out
+
+    def device_api_init_fill(self, n_streams: int, block_len: int, n_per_stream: int, dtype: str = "u32", stream=None):
+        """Streams initialised on the device by skip-ahead from this (one-stream) state: the library's example
+        kernel for prand_device_ops + prand_dev::Gen<GEN>::skipahead."""
+        import torch
+        tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[dtype]
+        out = torch.empty((n_per_stream, n_streams), dtype=tdt, device="cuda")
+        mant, log2 = split_dist(block_len)
+        _check(getattr(lib(), "prand_device_api_init_fill_" + dtype)(self._h, mant, log2, n_streams, out.data_ptr(),
+                                                                     n_per_stream, _stream_ptr(stream)),
+               "prand_device_api_init_fill")
         return out
 
     def generate_strided(self, n_per_stream: int, stride: int, dtype: str = "u32", stream=None):

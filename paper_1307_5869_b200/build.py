@@ -30,7 +30,7 @@ def _stale(target: str, deps: list[str]) -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     hdrs = [os.path.join(CSRC, h) for h in HEADERS]
     hdrs += [os.path.join(HERE, "..", "include", h)
-             for h in ("prand.h", "prand_host.h", "prand_device.cuh", "prand_device_gm.cuh")]
+             for h in ("prand.h", "prand_host.h", "prand_ops.h", "prand_device.cuh", "prand_device_gm.cuh")]
     hdrs.append(os.path.abspath(__file__))
     objdir = os.path.join(HERE, "build")
     os.makedirs(objdir, exist_ok=True)

@@ -5,22 +5,17 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 #include "../../include/prand.h"
+#include "../../include/prand_ops.h"
 
 namespace prand {
 
 enum { DT_U32 = 0, DT_F32 = 1, DT_F64 = 2 };
 
-// ---- skip operators (a0 builds them on the host, the kernels apply them) -------------------------
-// LFSR113: one step of a component is GF(2)-linear on its 32-bit word;
-// col[c][j] = image of the unit word 1<<j under the n-step map of component c.
-struct LfsrOp { uint32_t col[4][32]; };
-// MRG32K3A: A^n mod m1, B^n mod m2, row-major 3x3 residues.
-struct MrgOp { uint32_t a[9]; uint32_t b[9]; };
-// GM/GQ: n-th power of the companion matrix [[k,-q],[1,0]] mod g, row-major,
-// acting on the column (x^(n), x^(n-1)) = (xN, xP).
-struct GmOp { uint64_t m[4]; };
-// MT19937: g_v(x) = x^v mod phi(x) (eq. 10); bit (i & 31) of w[i >> 5] = a_i.
-struct MtOp { uint32_t w[624]; };
+// ---- skip operators (a0 builds them on the host, the kernels apply them): include/prand_ops.h --------
+typedef prand_lfsr113_op LfsrOp;
+typedef prand_mrg32k3a_op MrgOp;
+typedef prand_gm_op GmOp;
+typedef prand_mt19937_op MtOp;
 
 // GM/GQ parameters, Table 2 + Table 5 ensemble sizes.
 struct GmParams {
@@ -94,6 +89,10 @@ cudaError_t transpose_sections(cudaStream_t, const void *tmp, void *out, uint64_
 // one thread per stream through include/prand_device.cuh (example / self-test of the device API)
 cudaError_t devapi_generate(cudaStream_t, int gen, void *state, void *out, uint64_t ns, uint64_t n, int dtype,
                             LaunchInfo *);
+
+// device-side stream initialisation example: stream s = base stream skipped s * dist ahead with the table `ops`
+cudaError_t devapi_init_generate(cudaStream_t, int gen, const void *base, const void *ops, void *out, uint64_t ns,
+                                 uint64_t n, int dtype, LaunchInfo *);
 
 int sm_count();   // cached multiprocessor count of the current device
 

@@ -25,37 +25,11 @@ namespace {
 using namespace prand_dev;
 
 // ---- cold path: Barrett a*b mod g for the jump kernels ------------------------------------------
-struct Barrett { uint64_t g, mu; unsigned nb; };
-
-__device__ __forceinline__ uint64_t bmulmod(uint64_t a, uint64_t b, const Barrett &B)
-{
-    uint64_t lo = a * b, hi = __umul64hi(a, b);                      // x = a b < g^2 < 2^(2 nb)
-    uint64_t q1 = (hi << (65 - B.nb)) | (lo >> (B.nb - 1));          // x >> (nb-1) < 2^(nb+1)
-    uint64_t l2 = q1 * B.mu, h2 = __umul64hi(q1, B.mu);
-    uint64_t q3 = (h2 << (63 - B.nb)) | (l2 >> (B.nb + 1));          // floor(q1 mu / 2^(nb+1))
-    uint64_t r = lo - q3 * B.g;                                      // 0 <= x - q3 g < 3 g < 2^64
-    while (r >= B.g) r -= B.g;
-    return r;
-}
-__device__ __forceinline__ uint64_t baddmod(uint64_t a, uint64_t b, const Barrett &B)
-{
-    uint64_t t = a + b;                                              // < 2^62
-    return t >= B.g ? t - B.g : t;
-}
-// noinline: the generation kernels call it once per register-resident point (static indexing keeps
-// the ensemble out of local memory) and it is cold
-__device__ __noinline__ void gm_apply_bits(const GmOp *__restrict__ ops, uint64_t idx, uint64_t &xP,
-                                           uint64_t &xN, const Barrett &B)
-{
-    for (int lev = 0; idx != 0; lev++, idx >>= 1)
-        if (idx & 1) {
-            uint64_t m0 = __ldg(&ops[lev].m[0]), m1 = __ldg(&ops[lev].m[1]);
-            uint64_t m2 = __ldg(&ops[lev].m[2]), m3 = __ldg(&ops[lev].m[3]);
-            uint64_t n = baddmod(bmulmod(m0, xN, B), bmulmod(m1, xP, B), B);
-            uint64_t o = baddmod(bmulmod(m2, xN, B), bmulmod(m3, xP, B), B);
-            xN = n; xP = o;
-        }
-}
+// Barrett reduction mod g and the 2x2 skip are the device-callable API's (include/prand_device_gm.cuh)
+using prand_dev::Barrett;
+using prand_dev::bmulmod;
+using prand_dev::baddmod;
+using prand_dev::gm_apply_bits;
 
 // one thread per (stream, point)
 template <class W>

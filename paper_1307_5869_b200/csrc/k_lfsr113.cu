@@ -8,41 +8,15 @@
 // Jump-ahead: n steps are a GF(2)-linear map of the word, stored by columns (LfsrOp).
 // State layout (SoA): z[c * n_streams + s], c = 0..3.
 #include "k_common.cuh"
+#include "../../include/prand_device.cuh"
 
 namespace prand {
 namespace {
 
-template <int P, int Q, int S> __device__ __forceinline__ uint32_t tausworthe(uint32_t z)
-{
-    constexpr uint32_t kept = (0xFFFFFFFFu << (32 - P)) << S;   // (z & top_p) << s == (z << s) & kept
-    uint32_t b = ((z << Q) ^ z) >> (P - S);
-    return ((z << S) & kept) ^ b;
-}
-
-__device__ __forceinline__ uint32_t lfsr113_step(uint32_t (&z)[4])
-{
-    z[0] = tausworthe<31, 6, 18>(z[0]);
-    z[1] = tausworthe<29, 2, 2>(z[1]);
-    z[2] = tausworthe<28, 13, 7>(z[2]);
-    z[3] = tausworthe<25, 3, 13>(z[3]);
-    return z[0] ^ z[1] ^ z[2] ^ z[3];
-}
-
-__device__ __forceinline__ uint32_t gf2_matvec(const uint32_t *__restrict__ col, uint32_t z)
-{
-    uint32_t r = 0;
-#pragma unroll 8
-    for (int j = 0; j < 32; j++) r ^= (0u - ((z >> j) & 1u)) & __ldg(col + j);
-    return r;
-}
-
-__device__ __forceinline__ void lfsr113_apply_bits(const LfsrOp *__restrict__ ops, uint64_t idx,
-                                                   uint32_t (&z)[4])
-{
-    for (int lev = 0; idx != 0; lev++, idx >>= 1)
-        if (idx & 1)
-            for (int c = 0; c < 4; c++) z[c] = gf2_matvec(ops[lev].col[c], z[c]);
-}
+// the component step, the combined step and the GF(2) skip are the device-callable API's (one definition)
+using prand_dev::tausworthe;
+using prand_dev::lfsr113_step;
+using prand_dev::lfsr113_apply_bits;
 
 __global__ void __launch_bounds__(256)
 lfsr113_jump_kernel(const uint32_t *__restrict__ base, const uint32_t *st_in,

@@ -9,43 +9,19 @@
 // y_n, y_{n-1}, y_{n-2}.
 #include <cstdlib>
 #include "k_common.cuh"
+#include "../../include/prand_device.cuh"
 
 namespace prand {
 namespace {
 
-constexpr uint32_t M1 = 4294967087u, M2 = 4294944443u;
-constexpr uint32_t C1 = 209u, C2 = 22853u;
+// recurrences, reduction and the 3x3 skip are the device-callable API's (one definition of the arithmetic)
+constexpr uint32_t M1 = prand_dev::MRG_M1, M2 = prand_dev::MRG_M2, C1 = prand_dev::MRG_C1, C2 = prand_dev::MRG_C2;
+using prand_dev::mrg_next_x;
+using prand_dev::mrg_next_y;
 // small CTAs: with ~1000 CTAs on 148 SMs the most loaded SM is within 2% of the average
 constexpr int GEN_THREADS = 128;
 
-
 struct Mrg { uint32_t x0, x1, x2, y0, y1, y2; };   // x0 = x_n, x1 = x_{n-1}, x2 = x_{n-2}
-
-// x_{n+1} = (a x_{n-1} - b x_{n-2}) mod m1 from (x_{n-1}, x_{n-2}).  t = a x1 + b (m1 - x2) < 2^54,
-// t = hi 2^32 + lo; with the quotient estimate hi + 1:  t - (hi+1) m1 = lo + (hi+1) 209 - 2^32.
-// If the 32-bit addition carries the difference is the wrapped sum (< 2^30 < m1); otherwise the
-// estimate was one too large and adding m1 back gives sum - 209 in [0, m1).  Either way canonical.
-__device__ __forceinline__ uint32_t mrg_next_x(uint32_t x1, uint32_t x2, uint32_t c1)
-{
-    uint64_t t = (uint64_t)1403580u * x1 + (uint64_t)810728u * (M1 - x2);
-    uint32_t p = (uint32_t)(t >> 32) * c1 + c1;          // (hi + 1) * 209 < 2^30
-    uint32_t s = (uint32_t)t + p;
-    return s >= p ? s - C1 : s;                          // s >= p  <=>  no carry
-}
-// y_{n+1} = (c y_n - d y_{n-2}) mod m2 from (y_n, y_{n-2}).  One 64-bit fold u = hi 22853 + lo
-// (< 2^38, same residue; the carry chain keeps it out of a register pair), then the same
-// estimate-and-correct step on u = uh 2^32 + ul.
-__device__ __forceinline__ uint32_t mrg_next_y(uint32_t y0, uint32_t y2)
-{
-    uint64_t t = (uint64_t)527612u * y0 + (uint64_t)1370589u * (M2 - y2);
-    uint64_t f = (uint64_t)(uint32_t)(t >> 32) * C2;     // u = f + lo(t), kept as (uh + 1, ul)
-    uint32_t ul, uh1;
-    asm("add.cc.u32 %0, %2, %3;\n\taddc.u32 %1, %4, 1;"
-        : "=r"(ul), "=r"(uh1) : "r"((uint32_t)f), "r"((uint32_t)t), "r"((uint32_t)(f >> 32)));
-    uint32_t p = uh1 * C2;                               // (uh + 1) * 22853 < 2^21
-    uint32_t s = ul + p;
-    return s >= p ? s - C2 : s;
-}
 
 // Output of the combined generator from canonical x < m1, y < m2 < m1 (reading M1):
 // z = (x - y) mod m1 in [0, m1); the f64 map sends z = 0 to m1 (reading M3), i.e. z in [1, m1].
@@ -62,30 +38,10 @@ template <int DT> __device__ __forceinline__ typename OutElem<DT>::type mrg_outp
     }
 }
 
-// generic a*b mod m for the (cold) jump path: a, b < m = 2^32 - cfold
-__device__ __forceinline__ uint32_t mulmod32(uint32_t a, uint32_t b, uint32_t m, uint32_t cfold)
-{
-    uint64_t t = (uint64_t)a * b;
-    for (int k = 0; k < 3; k++) t = (t >> 32) * cfold + (uint32_t)t;   // < 2^32 + cfold after 3 folds
-    while (t >= m) t -= m;
-    return (uint32_t)t;
-}
-__device__ __forceinline__ uint32_t addmod32(uint32_t a, uint32_t b, uint32_t m)
-{
-    uint64_t t = (uint64_t)a + b;
-    return (uint32_t)(t >= m ? t - m : t);
-}
 __device__ __forceinline__ void matvec3(const uint32_t *__restrict__ mt, uint32_t &v0, uint32_t &v1,
                                         uint32_t &v2, uint32_t m, uint32_t cfold)
 {
-    uint32_t r[3];
-    for (int i = 0; i < 3; i++) {
-        uint32_t acc = mulmod32(__ldg(mt + 3 * i), v0, m, cfold);
-        acc = addmod32(acc, mulmod32(__ldg(mt + 3 * i + 1), v1, m, cfold), m);
-        acc = addmod32(acc, mulmod32(__ldg(mt + 3 * i + 2), v2, m, cfold), m);
-        r[i] = acc;
-    }
-    v0 = r[0]; v1 = r[1]; v2 = r[2];
+    prand_dev::mrg_matvec3(mt, v0, v1, v2, m, cfold);
 }
 __device__ __forceinline__ void mrg_apply_bits(const MrgOp *__restrict__ ops, uint64_t idx, Mrg &s)
 {

@@ -9,31 +9,22 @@
 // State layout: [stream][624] u32 (one stream's window is contiguous: a warp loads it coalesced).
 #include <cstdlib>
 #include "k_common.cuh"
+#include "../../include/prand_device.cuh"
 
 namespace prand {
 namespace {
 
 constexpr int NW = 624, MW = 397, DEG = 19937;
 
-__device__ __forceinline__ uint32_t mt_recur(uint32_t xi, uint32_t xi1, uint32_t xim)
-{
-    uint32_t y = (xi & 0x80000000u) | (xi1 & 0x7FFFFFFFu);
-    return xim ^ (y >> 1) ^ ((0u - (y & 1u)) & 0x9908B0DFu);
-}
+using prand_dev::mt_recur;
 
 // ---- eq. 10 in correlation form -----------------------------------------------------------------
-// One CTA per destination stream.  The source window is extended to x_0..x_{19937+623} in shared
-// memory (227 independent words per round), then output word j is the XOR of x_{i+j}
-// over the set coefficients a_i of g_v.  The coefficients are expanded, 2048 at a time, into a list of
-// set positions in shared memory, so that the accumulation loop has no bit scan and runs eight
-// positions (24 independent shared loads per thread) at a time; the list is padded with a position
-// whose words are zero.
-constexpr int APPLY_XWORDS = DEG + NW;                      // 20561
+// One CTA per destination stream runs the device-callable API's CTA-cooperative skip-ahead
+// (include/prand_device.cuh, mt19937_skipahead_cta: window extension + position-list accumulation).
+constexpr int APPLY_XWORDS = prand_dev::MT_SKIP_XWORDS;     // 20561
 constexpr int APPLY_ZERO = APPLY_XWORDS;                    // x[APPLY_ZERO .. +APPLY_ZPAD) = 0
-constexpr int APPLY_ZPAD = 771;                             // >= 768, makes the list 16-byte aligned
-constexpr int APPLY_CHUNK = 64;                             // polynomial words per expansion
-constexpr int APPLY_LIST = APPLY_CHUNK * 32 + 8;            // positions (u16) incl. padding
-constexpr size_t APPLY_SMEM = (size_t)(APPLY_XWORDS + APPLY_ZPAD) * sizeof(uint32_t) + APPLY_LIST * sizeof(uint16_t) + 16;
+constexpr int APPLY_ZPAD = prand_dev::MT_SKIP_ZPAD;
+constexpr size_t APPLY_SMEM = prand_dev::MT_SKIP_WORK_BYTES;
 
 // NT = 256: three output words per thread, two CTAs per SM (throughput: many streams); NT = 640: one
 // output word per thread, a third of the loads per thread (latency: the first levels of a doubling tree
@@ -47,77 +38,12 @@ __global__ void __launch_bounds__(NT)
 mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
                      uint64_t src_back, const MtOp *__restrict__ op)
 {
-    constexpr int APPLY_THREADS = NT, NOUT = NW / SPLIT, NO = (NOUT + NT - 1) / NT;
     static_assert(NW % SPLIT == 0, "SPLIT must divide 624");
-    const int out0 = (int)(blockIdx.x % SPLIT) * NOUT;
+    constexpr int NOUT = NW / SPLIT;
     extern __shared__ __align__(16) uint32_t smem[];
-    uint32_t *x = smem;                                                      // APPLY_XWORDS + APPLY_ZPAD
-    uint16_t *list = reinterpret_cast<uint16_t *>(smem + APPLY_XWORDS + APPLY_ZPAD);  // APPLY_LIST
-    int *meta = reinterpret_cast<int *>(list + APPLY_LIST);                  // [0] warp-0 total, [1] count
-    const int tid = threadIdx.x;
     const uint64_t dst = dst0 + blockIdx.x / SPLIT;
-    const uint32_t *src = st_src + (dst - src_back) * NW;
-    for (int j = tid; j < NW; j += APPLY_THREADS) x[j] = src[j];
-    for (int j = tid; j < APPLY_ZPAD; j += APPLY_THREADS) x[APPLY_ZERO + j] = 0;
-    __syncthreads();
-    constexpr int EXT = NT < NW - MW ? NT : NW - MW;       // at most 227 new words are independent
-    for (int r0 = 0; r0 < DEG; r0 += EXT) {
-        int k = r0 + tid;
-        if (tid < EXT && k < DEG) x[NW + k] = mt_recur(x[k], x[k + 1], x[k + MW]);
-        __syncthreads();
-    }
-    // thread t accumulates output words t, t + NT, ... (those below 624)
-    uint32_t acc[NO];
-    const uint32_t *xo[NO];
-#pragma unroll
-    for (int o = 0; o < NO; o++) {
-        acc[o] = 0;
-        xo[o] = x + (tid + NT * o < NOUT ? out0 + tid + NT * o : 0);
-    }
-    for (int c0 = 0; c0 < NW; c0 += APPLY_CHUNK) {
-        // expand polynomial words c0 .. c0+63 (threads 0..63, two warps) into the list of set positions
-        if (tid < APPLY_CHUNK) {
-            const int wi = c0 + tid;
-            uint32_t pw = wi < NW ? __ldg(&op->w[wi]) : 0u;
-            const int cnt = __popc(pw);
-            int incl = cnt;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-                if ((tid & 31) >= d) incl += v;
-            }
-            if (tid == 31) meta[0] = incl;
-            __syncwarp();
-            asm volatile("bar.sync 1, 64;" ::: "memory");
-            int pos = incl - cnt + (tid >= 32 ? meta[0] : 0);
-            if (tid == APPLY_CHUNK - 1) meta[1] = pos + cnt;
-            while (pw) {
-                list[pos++] = (uint16_t)(wi * 32 + (__ffs(pw) - 1));
-                pw &= pw - 1;
-            }
-        }
-        __syncthreads();
-        const int n = meta[1];
-        if (tid < 8) list[n + tid] = (uint16_t)APPLY_ZERO;
-        __syncthreads();
-        for (int k = 0; k < n; k += 8) {
-            const uint4 q = *reinterpret_cast<const uint4 *>(list + k);      // eight positions, uniform
-            const uint32_t ii[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-            for (int h = 0; h < 4; h++) {
-                const int ia = ii[h] & 0xFFFF, ib = ii[h] >> 16;
-#pragma unroll
-                for (int o = 0; o < NO; o++) acc[o] ^= xo[o][ia] ^ xo[o][ib];
-            }
-        }
-        __syncthreads();
-    }
-    uint32_t *d = st_dst + dst * NW;
-#pragma unroll
-    for (int o = 0; o < NO; o++) {
-        const int j = out0 + tid + NT * o;
-        if (tid + NT * o < NOUT) d[j] = j == 0 ? (acc[o] & 0x80000000u) : acc[o];   // only the top bit of word 0 is state (T2)
-    }
+    prand_dev::mt19937_skipahead_cta<NT, NOUT>(smem, op, st_src + (dst - src_back) * NW, st_dst + dst * NW,
+                                               (int)(blockIdx.x % SPLIT) * NOUT);
 }
 
 // Throughput form of the same application (many destination streams).  Thread t accumulates the four

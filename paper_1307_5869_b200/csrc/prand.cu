@@ -150,6 +150,7 @@ struct prand_state {
     bool host_ready;
     const char *last_kernel;
     cudaStream_t last_stream;   // stream of the most recent call: prand_free releases in its order
+    void *d_user_ops;       // prand_device_ops: operator table handed to the caller's kernels
     prand_state *sec;       // prand_generate_seq_*: cached family of sections (one stream per section)
     bool gm_clean;          // GM55/GQ58: every state word is a multiple of 2^t (true for states the
                             // library creates; an imported state is scanned), see k_gmgq.cu
@@ -365,6 +366,7 @@ void destroy(prand_state *st)
     if (st->host_ready) cudaStreamDestroy(st->copy_stream);
     if (st->d_ops) cudaFreeAsync(st->d_ops, s);
     if (st->d_chunk_ops) cudaFreeAsync(st->d_chunk_ops, s);
+    if (st->d_user_ops) cudaFreeAsync(st->d_user_ops, s);
     if (st->sec) { st->sec->last_stream = s; destroy(st->sec); }
     delete st;
 }
@@ -827,6 +829,58 @@ extern "C" void *prand_state_device_ptr(prand_state *st)
     return st ? st->d_state[st->cur] : nullptr;
 }
 extern "C" uint64_t prand_state_n_streams(const prand_state *st) { return st ? st->ns : 0; }
+
+extern "C" int prand_device_ops(prand_state *st, uint64_t dist_mant, unsigned dist_log2, unsigned levels,
+                                const void **d_ops, void *cuda_stream)
+{
+    if (!st || !d_ops || levels == 0 || levels > 64 || dist_log2 > 32768) return PRAND_ERR_ARG;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    st->last_stream = stream;
+    std::vector<unsigned char> ops;
+    int rc = build_level_ops(st->gen, Dist{dist_mant, dist_log2}, levels, ops);
+    if (rc) return rc;
+    if (st->d_user_ops) { CU(cudaFreeAsync(st->d_user_ops, stream)); st->d_user_ops = nullptr; }
+    CU(dev_alloc(&st->d_user_ops, ops.size(), stream));
+    UPLOAD(st->d_user_ops, ops.data(), ops.size(), stream);
+    CU(cudaStreamSynchronize(stream));                 // the host vector goes out of scope
+    *d_ops = st->d_user_ops;
+    return PRAND_OK;
+}
+
+namespace {
+int devapi_init_fill(prand_state *st, uint64_t mant, unsigned log2, uint64_t ns, void *out, uint64_t n, int dtype,
+                     cudaStream_t stream)
+{
+    if (!st || (!out && n) || ns == 0) return PRAND_ERR_ARG;
+    if (st->ns != 1) return PRAND_ERR_ARG;                 // the base stream
+    {
+        unsigned __int128 top = (unsigned __int128)(ns - 1) * mant;
+        if (top >> 64) return PRAND_ERR_OVERFLOW;
+    }
+    const void *ops = nullptr;
+    const unsigned levels = ns > 1 ? bit_length(ns - 1) : 1;
+    int rc = prand_device_ops(st, mant, log2, levels, &ops, stream);
+    if (rc) return rc;
+    if (n == 0) return PRAND_OK;
+    LaunchInfo li = {"", 0};
+    cudaError_t e = devapi_init_generate(stream, st->gen, st->d_state[st->cur], ops, out, ns, n, dtype, &li);
+    if (e != cudaSuccess) return cuda_fail(e);
+    note(st, li);
+    return PRAND_OK;
+}
+}  // namespace
+extern "C" int prand_device_api_init_fill_u32(prand_state *st, uint64_t m, unsigned l, uint64_t ns, uint32_t *out, uint64_t n, void *s)
+{
+    return devapi_init_fill(st, m, l, ns, out, n, DT_U32, (cudaStream_t)s);
+}
+extern "C" int prand_device_api_init_fill_f32(prand_state *st, uint64_t m, unsigned l, uint64_t ns, float *out, uint64_t n, void *s)
+{
+    return devapi_init_fill(st, m, l, ns, out, n, DT_F32, (cudaStream_t)s);
+}
+extern "C" int prand_device_api_init_fill_f64(prand_state *st, uint64_t m, unsigned l, uint64_t ns, double *out, uint64_t n, void *s)
+{
+    return devapi_init_fill(st, m, l, ns, out, n, DT_F64, (cudaStream_t)s);
+}
 
 namespace {
 int devapi_fill(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t stream)

@@ -6,6 +6,7 @@ stream on its own: each test generates the whole configuration on the GPU and co
 sample of streams (first, last, around CTA / warp boundaries, seeded random ones) plus the exported
 final states of those streams, bit for bit.  C1 is small enough to compare completely.
 """
+import ctypes as C
 import os
 import random
 
@@ -102,3 +103,38 @@ def test_c4_gm_f32_full_size_sampled(w):
 @pytest.mark.parametrize("w", workloads.C5, ids=lambda w: w.name)
 def test_c5_sweep_full_size_sampled(w):
     check_config(w, 6 if w.gen == "mt19937" else 40)
+
+
+@pytest.mark.parametrize("w", workloads.T7, ids=lambda w: w.name)
+def test_t7_sequence_fill_full_size_sampled_sections(w):
+    """The paper's Table 7 task at its size (one sequence, 2^29 doubles in device memory)
+    through prand_generate_seq_f64, in the section plan the bench times: ALL numbers of >= 16 sampled
+    sections (first, last, neighbours of the cuts, seeded random ones) against the serial oracle, the
+    elements on both sides of every sampled cut, and the state of the sequence after the fill."""
+    need_gpu(w.out_bytes + (6 << 30))
+    n = w.n_per_stream
+    S, L = C.c_uint64(), C.c_uint64()
+    assert P.lib().prand_host_plan_sections(P.gen_id(w.gen), n, C.byref(S), C.byref(L)) == 0
+    S, L = S.value, L.value
+    assert S > 16 and (S - 1) * L < n <= S * L
+    g = P.Generator(w.gen, w.seed, 1, 0)
+    g.jump(5)
+    out = g.generate_seq(n, w.dtype)
+    torch.cuda.synchronize()
+    kernel = g.last_kernel
+    st = g.state()
+    g.close()
+    assert "transpose" not in kernel, kernel              # written in place, no scratch pass
+    rng = random.Random(n ^ S)
+    picks = {0, 1, 2, S // 2 - 1, S // 2, S - 3, S - 2, S - 1}
+    while len(picks) < 16:
+        picks.add(rng.randrange(S))
+    base = oracle.State(w.gen, w.seed).jump(5)
+    for c in sorted(picks):
+        lo, hi = c * L, min(n, (c + 1) * L)
+        got = out[lo:hi].cpu().numpy().view(np.uint64)
+        want = base.copy().jump(lo).fill(hi - lo, w.dtype).view(np.uint64)
+        if not np.array_equal(got, want):
+            i = int(np.argmax(got != want))
+            raise AssertionError(f"{w.name} [{kernel}] section {c}: {(got != want).sum()} of {len(got)} differ, first at {i}")
+    assert st == base.copy().jump(n).export(), f"{w.name}: state after the fill differs"

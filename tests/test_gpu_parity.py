@@ -287,6 +287,26 @@ def test_device_callable_api_matches_oracle_and_bulk_kernels(gen):
 
 
 @pytest.mark.parametrize("gen", ALL_GENS)
+def test_device_side_init_by_skipahead_matches_prand_init(gen):
+    """PAPER.md:484-511 (rng_dev_init_sequence_ / rng_dev_skipahead_ over device constant tables): a
+    user-style kernel loads the base stream, skips s * block_len ahead with the table of
+    prand_device_ops and generates -- the numbers of the block-split family of prand_init."""
+    need_gpu()
+    seed = workloads.SEED.get(gen, 1)
+    ns, L = (6, 2**64) if gen == "mt19937" else (77, workloads.BLOCK_LEN[gen])
+    for dtype in (["u32", "f32", "f64"] if gen in ("mrg32k3a", "mt19937", "gm55") else ["u32"]):
+        g = P.Generator(gen, seed, 1, 0)
+        before = g.state()
+        got = g.device_api_init_fill(ns, L, 45, dtype).cpu().numpy().view(NPDT[dtype])
+        assert g.last_kernel == "devapi_init_example"
+        assert g.state() == before                      # the base stream is not modified
+        g.close()
+        w = Workload("devinit", gen, seed, ns, L, 45, dtype)
+        want, _ = oracle_run(w)
+        assert_same(w, got, want)
+
+
+@pytest.mark.parametrize("gen", ALL_GENS)
 def test_skip_per_step_generator(gen):
     """PAPER.md:226, Table 3: the sequence that outputs one number and jumps `stride` ahead."""
     need_gpu()
