@@ -59,6 +59,7 @@ _SIGS = {
     "prand_probe_pipe_count": (C.c_int, []),
     "prand_probe_pipe_name": (C.c_char_p, [C.c_int]),
     "prand_probe_pipe": (C.c_int, [C.c_int, C.c_uint64, C.POINTER(C.c_uint64), C.c_void_p]),
+    "prand_debug_set": (C.c_int, [C.c_char_p, C.c_char_p]),
     "prand_launch_count": (C.c_uint64, []),
     "prand_uploaded_bytes": (C.c_uint64, []),
     "prand_last_kernel": (C.c_char_p, [C.c_void_p]),
@@ -217,6 +218,11 @@ def prand_probe_pipe(op: int, iters: int, stream=None) -> int:
 
 def prand_probe_pipe_names() -> list[str]:
     return [lib().prand_probe_pipe_name(i).decode() for i in range(lib().prand_probe_pipe_count())]
+
+
+def prand_debug_set(name: str, value=None) -> None:
+    """Set (value) or clear (None) one test / tuning hook of the library (include/prand.h)."""
+    _check(lib().prand_debug_set(name.encode(), None if value is None else str(value).encode()), "prand_debug_set")
 
 
 def prand_launch_count() -> int:

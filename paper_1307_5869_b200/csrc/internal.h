@@ -60,6 +60,9 @@ struct GenArgs {
 struct LaunchInfo { const char *kernel; unsigned launches; };
 
 cudaError_t lfsr113_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
+// the paper's 128-table method: stream j advanced (idx0 + j * idx_stride) * mant * 2^log2,
+// one warp per stream; a.ops is not used
+cudaError_t lfsr113_table_jump(cudaStream_t, const JumpArgs &, uint64_t mant, unsigned log2, LaunchInfo *);
 cudaError_t lfsr113_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
 cudaError_t mrg32k3a_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
 cudaError_t mrg32k3a_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
@@ -94,6 +97,24 @@ cudaError_t devapi_generate(cudaStream_t, int gen, void *state, void *out, uint6
 cudaError_t devapi_init_generate(cudaStream_t, int gen, const void *base, const void *ops, void *out, uint64_t ns,
                                  uint64_t n, int dtype, LaunchInfo *);
 
-int sm_count();   // cached multiprocessor count of the current device
+int sm_count();   // multiprocessor count of the current device
+
+// Test / tuning hooks.  One process-wide struct, filled ONCE from the PRAND_* environment variables the
+// first time the library needs it and changed afterwards only through prand_debug_set (prand.h): the
+// launch paths read plain fields, never the environment.
+struct DebugHooks {
+    int mt_cfg;             // PRAND_MT_CFG: force an MT19937 generation kernel variant (-1: by stream count)
+    bool mt_apply_list;     // PRAND_MT_APPLY_LIST: the position-list application kernel at any size
+    int gm_lp;              // PRAND_GM_LP: lanes per GM61 stream (0: default)
+    int gm31_nf;            // PRAND_GM31_NF: GM31 points on the FP64 pipe (-1: default 14)
+    bool gm_watch_set;      // PRAND_GM_WATCH: limit of the optimistic steps' watch value
+    uint32_t gm_watch;
+    bool mrg_int;           // PRAND_MRG_INT: all-integer MRG32K3A kernel for 4-byte outputs
+    bool gm_init_matrix;    // PRAND_GM_INIT=matrix: one matrix jump per stream instead of the eq.-2 tree
+    uint64_t chunk_len;     // PRAND_CHUNK_LEN: force the sub-section length (0: plan_chunks decides)
+    bool lfsr_table;        // PRAND_LFSR_INIT=table: the paper's 128-table jump method for LFSR113
+    bool mt_host_poly;      // PRAND_MT_POLY=host: compute every MT19937 jump polynomial on the host (no table)
+};
+const DebugHooks &debug_hooks();
 
 }  // namespace prand

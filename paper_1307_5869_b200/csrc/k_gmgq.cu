@@ -317,8 +317,7 @@ template <int NF> cudaError_t launch_gm31_hybrid(cudaStream_t stream, const GenA
 template <class Tr> uint32_t gm_watch_limit()
 {
     if constexpr (Tr::HAS_FAST) {
-        if (const char *env = std::getenv("PRAND_GM_WATCH")) return (uint32_t)std::strtoul(env, nullptr, 0);
-        return Tr::WATCH_LIMIT;
+        return debug_hooks().gm_watch_set ? debug_hooks().gm_watch : Tr::WATCH_LIMIT;
     } else {
         return 0xFFFFFFFFu;
     }
@@ -399,14 +398,12 @@ cudaError_t gm_generate(cudaStream_t stream, int gen, const GenArgs &a, LaunchIn
     if (!p) return cudaErrorInvalidValue;
     Barrett B = barrett_of(p);
     li->launches = 1;
-    int lp = 0;                                              // test / tuning hook: lanes per stream
-    if (const char *env = std::getenv("PRAND_GM_LP")) lp = std::atoi(env);
+    const int lp = debug_hooks().gm_lp;                      // test / tuning hook: lanes per stream
     switch (gen) {
     case PRAND_GM19: li->kernel = "gm19_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM19>, 1>(stream, a, B);
     case PRAND_GM29: li->kernel = "gm29_gen<LP=1>"; return dispatch_dt<Gm<PRAND_GM29>, 1>(stream, a, B);
     case PRAND_GM31: {
-        int nf = 14;                                         // points on the FP64 pipe (test / tuning hook)
-        if (const char *env = std::getenv("PRAND_GM31_NF")) nf = std::atoi(env);
+        const int nf = debug_hooks().gm31_nf < 0 ? 14 : debug_hooks().gm31_nf;   // points on the FP64 pipe (test / tuning hook)
         if (nf == 12) { li->kernel = "gm31_gen<fp64 x12>"; return launch_gm31_hybrid<12>(stream, a, B); }
         if (nf == 14) { li->kernel = "gm31_gen<fp64 x14>"; return launch_gm31_hybrid<14>(stream, a, B); }
         if (nf == 16) { li->kernel = "gm31_gen<fp64 x16>"; return launch_gm31_hybrid<16>(stream, a, B); }

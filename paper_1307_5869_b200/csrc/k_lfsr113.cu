@@ -31,6 +31,76 @@ lfsr113_jump_kernel(const uint32_t *__restrict__ base, const uint32_t *st_in,
     for (int c = 0; c < 4; c++) st_out[c * ns + s] = z[c];
 }
 
+// ---- the paper's own jump algorithm (section 5.3) as an alternate --------------------
+// By eq. 9 the sequence decimated by k = 2^e, y_l = x_{kl}, obeys the recurrence (7) itself.  A "table"
+// starts from p consecutive bits, extends them to 2p - 1 with (7) (the row x_{2^n p} .. x_{2^n (2p-1)} of the
+// paper) and keeps every second bit: after n rounds it holds x_0, x_{2^n}, ..., x_{(p-1) 2^n}, and bit s of
+// it is x_{s 2^n}, the first bit of the output word 2^n steps ahead (eq. 8).  Bit i of that word comes from
+// the table started at x_i: 32 tables per component, 128 per stream -- "constructed independently using
+// different threads": one warp per stream, lane = start bit, each lane runs its four components; the new
+// state words are assembled with a warp ballot.  A jump by E 2^b outputs is the succession of the jumps
+// 2^(i + b) over the set bits i of E.  Words are kept MSB first (bit 63 - k of a 64-bit register = x_k).
+template <int P, int Q, int S> __device__ __forceinline__ uint32_t tausworthe_table_bit(uint32_t z, int lane, unsigned n);
+
+__device__ __forceinline__ uint64_t keep_even_msb_first(uint64_t y)
+{
+    y &= 0xAAAAAAAAAAAAAAAAull;                           // indices 0, 2, 4, ... (MSB first) = odd bit positions
+    y = (y | (y << 1)) & 0xCCCCCCCCCCCCCCCCull;
+    y = (y | (y << 2)) & 0xF0F0F0F0F0F0F0F0ull;
+    y = (y | (y << 4)) & 0xFF00FF00FF00FF00ull;
+    y = (y | (y << 8)) & 0xFFFF0000FFFF0000ull;
+    y = (y | (y << 16)) & 0xFFFFFFFF00000000ull;
+    return y;
+}
+// (v, valid): the top `valid` bits of v are sequence bits; extend to `target` bits with eq. 7
+template <int P, int Q> __device__ __forceinline__ uint64_t taus_extend(uint64_t v, int valid, int target)
+{
+    while (valid < target) {
+        int g = (P - Q < target - valid) ? P - Q : target - valid;
+        uint64_t t = (v >> P) ^ (v >> (P - Q));          // bit index i holds x_{i-P} ^ x_{i-P+Q}
+        uint64_t m = (~0ull >> valid) & ~((valid + g >= 64) ? 0ull : (~0ull >> (valid + g)));
+        v |= t & m;
+        valid += g;
+    }
+    return v;
+}
+template <int P, int Q, int S> __device__ __forceinline__ uint32_t tausworthe_table_bit(uint32_t z, int lane, unsigned n)
+{
+    constexpr uint32_t top_p = 0xFFFFFFFFu << (32 - P);
+    constexpr uint64_t top_p64 = ~0ull << (64 - P);
+    uint64_t y = taus_extend<P, Q>((uint64_t)(z & top_p) << 32, P, 64) << lane;    // the table's p start bits x_lane ..
+    y &= top_p64;
+    for (unsigned r = 0; r < n; r++) y = keep_even_msb_first(taus_extend<P, Q>(y, P, 2 * P - 1)) & top_p64;
+    return (uint32_t)(y >> (63 - S)) & 1u;
+}
+
+constexpr int TABLE_WARPS = 4;
+__global__ void __launch_bounds__(32 * TABLE_WARPS)
+lfsr113_table_jump_kernel(const uint32_t *__restrict__ base, const uint32_t *st_in, uint32_t *st_out, uint64_t ns,
+                          uint64_t mant, unsigned log2, uint64_t idx0, uint64_t idx_stride)
+{
+    const uint64_t s = (uint64_t)blockIdx.x * TABLE_WARPS + (threadIdx.x >> 5);
+    if (s >= ns) return;                                    // whole warp
+    const int lane = threadIdx.x & 31;
+    uint32_t z[4];
+    for (int c = 0; c < 4; c++) z[c] = base ? base[c] : st_in[c * ns + s];
+    uint64_t e = (idx0 + s * idx_stride) * mant;            // the launcher guarantees no overflow
+    for (unsigned i = 0; e != 0; i++, e >>= 1) {
+        if (!(e & 1)) continue;
+        const unsigned n = i + log2;                        // jump 2^n outputs
+        const uint32_t b0 = tausworthe_table_bit<31, 6, 18>(z[0], lane, n);
+        const uint32_t b1 = tausworthe_table_bit<29, 2, 2>(z[1], lane, n);
+        const uint32_t b2 = tausworthe_table_bit<28, 13, 7>(z[2], lane, n);
+        const uint32_t b3 = tausworthe_table_bit<25, 3, 13>(z[3], lane, n);
+        // lane i holds bit x_{s 2^n + i} = bit 31 - i of the new word
+        z[0] = __brev(__ballot_sync(0xFFFFFFFFu, b0));
+        z[1] = __brev(__ballot_sync(0xFFFFFFFFu, b1));
+        z[2] = __brev(__ballot_sync(0xFFFFFFFFu, b2));
+        z[3] = __brev(__ballot_sync(0xFFFFFFFFu, b3));
+    }
+    if (lane < 4) st_out[lane * ns + s] = lane == 0 ? z[0] : lane == 1 ? z[1] : lane == 2 ? z[2] : z[3];
+}
+
 // ---- bit-stream form of one component (hot path) -------------------------------------------------
 // Successive output words of a component overlap: word n is bits x_{ns}..x_{ns+31} of ONE bit
 // sequence, so an output consumes only s fresh bits (18 + 2 + 7 + 13 = 40 for the four components)
@@ -232,6 +302,17 @@ cudaError_t lfsr113_jump(cudaStream_t stream, const JumpArgs &a, LaunchInfo *li)
                                                     (uint32_t *)a.st_out, a.n_streams,
                                                     (const LfsrOp *)a.ops, a.idx0, a.idx_stride);
     li->kernel = "lfsr113_jump";
+    li->launches = 1;
+    return cudaGetLastError();
+}
+
+cudaError_t lfsr113_table_jump(cudaStream_t stream, const JumpArgs &a, uint64_t mant, unsigned log2, LaunchInfo *li)
+{
+    unsigned blocks = (unsigned)ceil_div_u64(a.n_streams, TABLE_WARPS);
+    lfsr113_table_jump_kernel<<<blocks, 32 * TABLE_WARPS, 0, stream>>>((const uint32_t *)a.base, (const uint32_t *)a.st_in,
+                                                                      (uint32_t *)a.st_out, a.n_streams, mant, log2,
+                                                                      a.idx0, a.idx_stride);
+    li->kernel = "lfsr113_table_jump";
     li->launches = 1;
     return cudaGetLastError();
 }

@@ -359,7 +359,7 @@ template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenAr
     typedef typename OutElem<DT>::type T;
     const uint64_t groups = a.n_streams / V;
     dim3 grid((unsigned)ceil_div_u64(groups, GEN_THREADS), (unsigned)a.n_chunks);
-    const bool int_only = std::getenv("PRAND_MRG_INT") != nullptr;     // test hook: integer y component
+    const bool int_only = debug_hooks().mrg_int;                       // test hook: integer y component
     if (DT != DT_F64 && !int_only)
         mrg32k3a_gen_fp64y_kernel<V, DT><<<grid, GEN_THREADS, 0, stream>>>(
             (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (T *)a.out, a.n_streams, a.n, a.chunk_len,

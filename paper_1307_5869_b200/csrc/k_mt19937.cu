@@ -1020,7 +1020,7 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
         mt19937_apply_kernel<160, 4><<<(unsigned)(4 * count), 160, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     else if (count <= (uint64_t)sm_count())
         mt19937_apply_kernel<640, 1><<<(unsigned)count, 640, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    else if (std::getenv("PRAND_MT_APPLY_LIST"))             // test hook: the position-list kernel at any size
+    else if (debug_hooks().mt_apply_list)                    // test hook: the position-list kernel at any size
         mt19937_apply_kernel<256, 1><<<(unsigned)count, 256, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     else
         mt19937_apply_win_kernel<<<(unsigned)count, APPLYW_THREADS, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
@@ -1052,8 +1052,8 @@ cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *
     const bool gather_ok = a.dtype != DT_F64 && a.n_streams % 4 == 0 && (uintptr_t)a.out % 16 == 0 && a.n / NW < (1ull << 32);
     // (not the default: measured 1.29 ms on C3 against 1.00 ms for the cluster-pair kernel -- the exchange is
     // bound by the ~10-13 B/clk/SM that distributed shared memory moves between four CTAs)
-    if (const char *env = std::getenv("PRAND_MT_CFG")) {                      // test hook: force a variant
-        const int want = std::atoi(env);
+    if (debug_hooks().mt_cfg >= 0) {                                          // test hook: force a variant
+        const int want = debug_hooks().mt_cfg;
         if (want != 3 || gather_ok) cfg = want;
     }
     switch (cfg) {

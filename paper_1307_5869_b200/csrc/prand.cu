@@ -5,6 +5,7 @@
 #include <atomic>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -47,16 +48,44 @@ const GmParams *gm_params(int gen)
 
 int sm_count()
 {
-    static int cached_dev = -1, cached = 0;
-    int dev = 0;
+    // per device, no shared mutable cache: the attribute query costs well under a microsecond
+    int dev = 0, n = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-    if (dev != cached_dev) {
-        int n = 0;
-        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
-        cached = n;
-        cached_dev = dev;
-    }
-    return cached;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    return n;
+}
+
+namespace {
+std::mutex g_hooks_mu;
+DebugHooks g_hooks;
+std::once_flag g_hooks_once;
+
+void hook_assign(DebugHooks &h, const std::string &name, const char *v)
+{
+    const bool on = v && *v;
+    if (name == "PRAND_MT_CFG") h.mt_cfg = on ? std::atoi(v) : -1;
+    else if (name == "PRAND_MT_APPLY_LIST") h.mt_apply_list = on;
+    else if (name == "PRAND_GM_LP") h.gm_lp = on ? std::atoi(v) : 0;
+    else if (name == "PRAND_GM31_NF") h.gm31_nf = on ? std::atoi(v) : -1;
+    else if (name == "PRAND_GM_WATCH") { h.gm_watch_set = on; h.gm_watch = on ? (uint32_t)std::strtoul(v, nullptr, 0) : 0; }
+    else if (name == "PRAND_MRG_INT") h.mrg_int = on;
+    else if (name == "PRAND_GM_INIT") h.gm_init_matrix = on && std::string(v) == "matrix";
+    else if (name == "PRAND_CHUNK_LEN") h.chunk_len = on ? std::strtoull(v, nullptr, 10) : 0;
+    else if (name == "PRAND_LFSR_INIT") h.lfsr_table = on && std::string(v) == "table";
+    else if (name == "PRAND_MT_POLY") h.mt_host_poly = on && std::string(v) == "host";
+}
+const char *const HOOK_NAMES[] = {"PRAND_MT_CFG", "PRAND_MT_APPLY_LIST", "PRAND_GM_LP", "PRAND_GM31_NF", "PRAND_GM_WATCH",
+                                  "PRAND_MRG_INT", "PRAND_GM_INIT", "PRAND_CHUNK_LEN", "PRAND_LFSR_INIT", "PRAND_MT_POLY"};
+void hooks_from_env()
+{
+    for (const char *n : HOOK_NAMES) hook_assign(g_hooks, n, std::getenv(n));
+}
+}  // namespace
+
+const DebugHooks &debug_hooks()
+{
+    std::call_once(g_hooks_once, hooks_from_env);
+    return g_hooks;
 }
 
 }  // namespace prand
@@ -236,8 +265,12 @@ int build_seed_state(int gen, uint64_t seed, std::vector<unsigned char> &bytes)
     return PRAND_OK;
 }
 
-cudaError_t launch_jump(cudaStream_t stream, int gen, const JumpArgs &a, LaunchInfo *li)
+// dist != nullptr: the distance the level-0 operator of a.ops stands for (the LFSR113 table method works
+// from the distance itself)
+cudaError_t launch_jump(cudaStream_t stream, int gen, const JumpArgs &a, LaunchInfo *li, const Dist *dist = nullptr)
 {
+    if (gen == PRAND_LFSR113 && dist && debug_hooks().lfsr_table)
+        return lfsr113_table_jump(stream, a, dist->mant, dist->log2, li);
     if (gen == PRAND_LFSR113) return lfsr113_jump(stream, a, li);
     if (gen == PRAND_MRG32K3A) return mrg32k3a_jump(stream, a, li);
     return gm_jump(stream, gen, a, li);
@@ -324,12 +357,11 @@ int init_body(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream, const
     // GM/GQ with many streams: the paper's own relation (eq. 2-3) fills the family.
     // Streams 0 and 1 come from the jump kernel; then, level by level, stream s = k_n stream(s - 2^j)
     // - q_n stream(s - 2^(j+1)) with n = 2^j L -- two modular products per state word instead of one
-    // matrix product per set bit of s.  PRAND_GM_INIT=matrix keeps the matrix path (test hook).
-    const bool tree = is_gm(st->gen) && st->ns >= 64 && !(std::getenv("PRAND_GM_INIT") &&
-                                                          std::string(std::getenv("PRAND_GM_INIT")) == "matrix");
+    // matrix product per set bit of s.  the hook PRAND_GM_INIT=matrix keeps the matrix path.
+    const bool tree = is_gm(st->gen) && st->ns >= 64 && !debug_hooks().gm_init_matrix;
     LaunchInfo li;
     if (!tree) {
-        CU(launch_jump(stream, st->gen, a, &li));
+        CU(launch_jump(stream, st->gen, a, &li, &L));
         note(st, li);
         return PRAND_OK;
     }
@@ -439,7 +471,7 @@ int jump_prepare(prand_state *st, Dist n, cudaStream_t stream)
     return PRAND_OK;
 }
 // apply the operator in st->d_ops to every stream
-int jump_launch(prand_state *st, cudaStream_t stream)
+int jump_launch(prand_state *st, cudaStream_t stream, const Dist *dist = nullptr)
 {
     LaunchInfo li;
     if (st->gen == PRAND_MT19937) {
@@ -455,7 +487,7 @@ int jump_launch(prand_state *st, cudaStream_t stream)
         a.idx0 = 1;                          // every stream applies level 0 exactly once
         a.idx_stride = 0;
         a.count = 0;
-        CU(launch_jump(stream, st->gen, a, &li));
+        CU(launch_jump(stream, st->gen, a, &li, dist));
     }
     note(st, li);
     return PRAND_OK;
@@ -472,7 +504,7 @@ extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_l
     Dist n = {steps_mant, steps_log2};
     int rc = jump_prepare(st, n, stream);
     if (rc) return rc;
-    rc = jump_launch(st, stream);
+    rc = jump_launch(st, stream, &n);
     if (rc) return rc;
     if (steps_log2 >= 4 || steps_mant >= 16) st->gm_clean = true;   // past the 2-adic transient
     return PRAND_OK;
@@ -492,8 +524,7 @@ void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t 
     *chunk_len = n;
     *n_chunks = 1;
     if (gen == PRAND_MT19937 || n == 0) return;
-    uint64_t forced = 0;
-    if (const char *env = std::getenv("PRAND_CHUNK_LEN")) forced = std::strtoull(env, nullptr, 10);
+    const uint64_t forced = debug_hooks().chunk_len;
     uint64_t len;
     if (forced) {
         len = forced;
@@ -1002,6 +1033,18 @@ extern "C" int prand_fill_u32(uint32_t *out, uint64_t n_words, uint32_t value, v
     LaunchInfo li = {"", 0};
     CU(fill_u32((cudaStream_t)cuda_stream, out, n_words, value, &li));
     note(nullptr, li);
+    return PRAND_OK;
+}
+
+extern "C" int prand_debug_set(const char *name, const char *value)
+{
+    if (!name) return PRAND_ERR_ARG;
+    bool known = false;
+    for (const char *n : HOOK_NAMES) known = known || std::string(n) == name;
+    if (!known) return PRAND_ERR_ARG;
+    debug_hooks();                                         // environment first, once
+    std::lock_guard<std::mutex> lock(g_hooks_mu);
+    hook_assign(g_hooks, name, value);
     return PRAND_OK;
 }
 

@@ -96,7 +96,7 @@ def test_mt19937_every_kernel_configuration(cfg, monkeypatch):
     gather) variant of the MT19937 generation kernel, over whole rounds of 624, several rounds and
     ragged tails, with stream counts that leave CTAs partly or wholly dead."""
     need_gpu()
-    monkeypatch.setenv("PRAND_MT_CFG", str(cfg))
+    P.prand_debug_set("PRAND_MT_CFG", str(cfg))
     cases = [(5, [624, 1248, 1, 700], "u32"), (13, [2048], "f32"), (8, [1500, 623], "f64"), (70, [209, 1300], "u32")]
     if cfg == 3:      # the cluster-gather kernel takes 4-byte outputs and stream counts that are multiples of 4
         cases = [(4, [624, 1248, 1, 700], "u32"), (12, [2048], "f32"), (16, [1500, 623, 3000], "u32"),
@@ -108,7 +108,7 @@ def test_mt19937_every_kernel_configuration(cfg, monkeypatch):
         want, wst = oracle_run(w)
         assert_same(w, got, want)
         assert st == wst, f"cfg {cfg}: exported states differ"
-    monkeypatch.delenv("PRAND_MT_CFG")
+    P.prand_debug_set("PRAND_MT_CFG", None)
 
 
 @pytest.mark.parametrize("gen", ALL_GENS)
@@ -143,11 +143,11 @@ def test_sub_section_chunking_changes_nothing(gen, monkeypatch):
     w = Workload("chunked", gen, workloads.SEED.get(gen, 1), 44, workloads.BLOCK_LEN[gen], 203, "f32")
     want, wst = oracle_run(w)
     for chunk in (4, 8, 52, 200):
-        monkeypatch.setenv("PRAND_CHUNK_LEN", str(chunk))
+        P.prand_debug_set("PRAND_CHUNK_LEN", str(chunk))
         got, st, _ = lib_run(w, calls=[150, 53])
         assert_same(w, got, want)
         assert st == wst
-    monkeypatch.delenv("PRAND_CHUNK_LEN")
+    P.prand_debug_set("PRAND_CHUNK_LEN", None)
 
 
 @pytest.mark.parametrize("gen", ["lfsr113", "mrg32k3a", "mt19937", "gm29", "gm61", "gq58.3"])
@@ -286,6 +286,31 @@ def test_device_callable_api_matches_oracle_and_bulk_kernels(gen):
         assert st == wst
 
 
+def test_lfsr113_table_method_equals_matrix_jumps_and_oracle():
+    """PAPER.md:363-370 (section 5.3): the paper's own jump algorithm for LFSR113 -- 128 tables per stream
+    built by eq. 9, one warp per stream -- as an alternate of the GF(2) matrix path (PRAND_LFSR_INIT=table):
+    stream initialisation by block splitting and prand_jump must reach the same states."""
+    need_gpu()
+    for ns, L, jump in [(70, 2**40, 12345), (33, 3 * 2**33, 5 << 40), (5, 1, 1), (130, 777, 0)]:
+        w = Workload("lfsr-table", "lfsr113", 12345, ns, L, 40, "u32")
+        ref, rst, _ = lib_run(w, pre_jump=jump)
+        P.prand_debug_set("PRAND_LFSR_INIT", "table")
+        try:
+            g = P.Generator("lfsr113", 12345, ns, L)
+            assert g.last_kernel == "lfsr113_table_jump"
+            if jump:
+                g.jump(jump)
+                assert g.last_kernel == "lfsr113_table_jump"
+            got = g.generate(40, "u32").cpu().numpy().view(np.uint32)
+            st = g.state()
+            g.close()
+        finally:
+            P.prand_debug_set("PRAND_LFSR_INIT", None)
+        want, wst = oracle_run(w, pre_jump=jump)
+        assert_same(w, got, want)
+        assert np.array_equal(got, ref) and st == rst == wst
+
+
 @pytest.mark.parametrize("gen", ALL_GENS)
 def test_device_side_init_by_skipahead_matches_prand_init(gen):
     """PAPER.md:484-511 (rng_dev_init_sequence_ / rng_dev_skipahead_ over device constant tables): a
@@ -335,16 +360,16 @@ def test_optimistic_steps_fall_back_exactly(gen, limit, monkeypatch):
     the watched limb reaches a limit (probability ~2^-28 in production).  Lowering the limit makes the
     fallback run always ("0") or for a quarter of the points: the numbers must not change."""
     need_gpu()
-    monkeypatch.setenv("PRAND_GM_WATCH", limit)
+    P.prand_debug_set("PRAND_GM_WATCH", limit)
     for lp in ("1", "4") if gen == "gm61" else ("1",):
-        monkeypatch.setenv("PRAND_GM_LP", lp)
+        P.prand_debug_set("PRAND_GM_LP", lp)
         w = Workload("watch", gen, 1, 70, workloads.BLOCK_LEN[gen], 37, "u32")
         got, st, _ = lib_run(w, calls=[20, 17])
         want, wst = oracle_run(w)
         assert_same(w, got, want)
         assert st == wst
-    monkeypatch.delenv("PRAND_GM_WATCH")
-    monkeypatch.delenv("PRAND_GM_LP")
+    P.prand_debug_set("PRAND_GM_WATCH", None)
+    P.prand_debug_set("PRAND_GM_LP", None)
 
 
 @pytest.mark.parametrize("dtype", ["u32", "f32"])
@@ -357,11 +382,11 @@ def test_mrg32k3a_integer_and_fp64_pipe_kernels_agree_with_the_oracle(dtype, mon
     want, wst = oracle_run(w)
     for hook in (None, "1"):
         if hook:
-            monkeypatch.setenv("PRAND_MRG_INT", hook)
+            P.prand_debug_set("PRAND_MRG_INT", hook)
         got, st, _ = lib_run(w, calls=[100, 103])
         assert_same(w, got, want)
         assert st == wst
-    monkeypatch.delenv("PRAND_MRG_INT", raising=False)
+    P.prand_debug_set("PRAND_MRG_INT", None)
 
 
 @pytest.mark.parametrize("gen", ["gm19", "gm31", "gm55", "gm61", "gq58.1", "gq58.3"])
@@ -376,12 +401,12 @@ def test_gm_family_init_by_the_papers_relation_equals_matrix_jumps(gen, monkeypa
         st_tree = g.state()
         assert g.last_kernel == "gm_tree"
         g.close()
-        monkeypatch.setenv("PRAND_GM_INIT", "matrix")
+        P.prand_debug_set("PRAND_GM_INIT", "matrix")
         g = P.Generator(gen, 1, ns, L, first_stream=first)
         st_mat = g.state()
         assert g.last_kernel == "gm_jump"
         g.close()
-        monkeypatch.delenv("PRAND_GM_INIT")
+        P.prand_debug_set("PRAND_GM_INIT", None)
         assert st_tree == st_mat, f"{gen}: tree init differs from matrix init (first {first}, ns {ns})"
     _, wst = oracle.streams(gen, 1, 5, 777, L, 0, "u32", threads=CPU_THREADS)
     assert st_tree[:0] == b"" and P.Generator(gen, 1, 777, L, first_stream=5).state() == wst.tobytes()
@@ -392,14 +417,14 @@ def test_gm31_points_on_the_fp64_pipe_are_exact(nf, monkeypatch):
     """GM31 steps 14 of its 32 points in double precision on the FP64 pipe (exact floor division by
     2^31 - 1); PRAND_GM31_NF selects other splits (0: all points on the integer pipes)."""
     need_gpu()
-    monkeypatch.setenv("PRAND_GM31_NF", nf)
+    P.prand_debug_set("PRAND_GM31_NF", nf)
     w = Workload("gm31-fp64", "gm31", 1, 300, workloads.BLOCK_LEN["gm31"], 101, "u32")
     got, st, kernel = lib_run(w, calls=[50, 51])
     want, wst = oracle_run(w)
     assert_same(w, got, want)
     assert st == wst
     assert ("fp64" in kernel) == (nf != "0")
-    monkeypatch.delenv("PRAND_GM31_NF")
+    P.prand_debug_set("PRAND_GM31_NF", None)
 
 
 def got_dtype(dtype):
