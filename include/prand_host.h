@@ -37,6 +37,15 @@ int prand_host_mt19937_phi(uint32_t *words624);
 int prand_host_mt19937_mulmod(const uint32_t *a624, const uint32_t *b624, uint32_t *r624);
 
 /*
+ * PRAND ships the MT19937 jump polynomials x^v mod phi for v = 2^n (n = 0..511) and
+ * v = m 2^i (m = 15..24, i = 0..127) precomputed; libprand's build step writes the same table
+ * (csrc/mt_table_gen.cpp -> mt19937_polys.bin next to the library).  Copies the record of
+ * v = mant * 2^log2 (624 u32 words, layout of prand_mt19937_op) or returns PRAND_ERR_ARG if v is not of a
+ * tabulated form or the table file is missing.
+ */
+int prand_host_mt19937_table(uint64_t mant, unsigned log2, uint32_t *words624);
+
+/*
  * Launch policy of prand_generate_* on a device with `sm_count` multiprocessors: a stream's range
  * of n_per_stream outputs is cut into n_chunks sub-sections of chunk_len reached by jump-ahead
  * when there are too few streams to fill the GPU.  dtype: 0 u32, 1 f32, 2 f64.

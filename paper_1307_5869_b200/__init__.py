@@ -73,6 +73,7 @@ _SIGS = {
     "prand_host_seed_state": (C.c_int, [C.c_int, C.c_uint64, C.c_void_p, C.c_size_t]),
     "prand_host_mt19937_phi": (C.c_int, [C.c_void_p]),
     "prand_host_mt19937_mulmod": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
+    "prand_host_mt19937_table": (C.c_int, [C.c_uint64, C.c_uint, C.c_void_p]),
     "prand_host_gm_kq": (C.c_int, [C.c_int, C.c_uint64, C.c_uint, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
     "prand_host_plan_sections": (C.c_int, [C.c_int, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
     "prand_host_plan": (C.c_int, [C.c_int, C.c_uint64, C.c_uint64, C.c_int, C.c_int,
@@ -259,6 +260,14 @@ def prand_host_mt19937_phi() -> bytes:
     buf = C.create_string_buffer(624 * 4)
     _check(lib().prand_host_mt19937_phi(buf), "prand_host_mt19937_phi")
     return buf.raw
+
+
+def prand_host_mt19937_table(dist: int):
+    """The precomputed polynomial of x^dist as bytes, or None if dist is not tabulated."""
+    mant, log2 = split_dist(dist)
+    buf = C.create_string_buffer(624 * 4)
+    rc = lib().prand_host_mt19937_table(mant, log2, buf)
+    return buf.raw if rc == 0 else None
 
 
 def prand_host_mt19937_mulmod(a: bytes, b: bytes) -> bytes:

@@ -12,6 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libprand.so")
+MT_TABLE = os.path.join(HERE, "mt19937_polys.bin")
 SOURCES = ["prand.cu", "skip_ops.cpp", "k_lfsr113.cu", "k_mrg32k3a.cu", "k_mt19937.cu", "k_gmgq.cu",
            "k_fill.cu", "k_devapi.cu", "k_probe.cu"]
 HEADERS = ["internal.h", "k_common.cuh", "skip_ops.h"]
@@ -57,7 +58,24 @@ def build(force: bool = False, verbose: bool = False) -> str:
         tmp = LIB + f".tmp{os.getpid()}"
         subprocess.check_call([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + objs + ["-cudart", "shared"])
         os.replace(tmp, LIB)
+    build_mt_table(force)
     return LIB
+
+
+def build_mt_table(force: bool = False) -> str:
+    """The MT19937 jump-polynomial table of PAPER.md:378 (x^v mod phi for v = 2^n, n < 512, and v = m 2^i,
+    m = 15..24, i < 128; 1792 x 2496 bytes): written once by csrc/mt_table_gen.cpp next to the library."""
+    srcs = [os.path.join(CSRC, f) for f in ("mt_table_gen.cpp", "skip_ops.cpp")]
+    deps = srcs + [os.path.join(CSRC, f) for f in ("skip_ops.h", "internal.h")]
+    if not force and not _stale(MT_TABLE, deps):
+        return MT_TABLE
+    exe = os.path.join(HERE, "build", "mt_table_gen")
+    subprocess.check_call([NVCC, "-O2", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-x", "cu"] + srcs +
+                          ["-o", exe, "-cudart", "shared"])
+    tmp = MT_TABLE + f".tmp{os.getpid()}"
+    subprocess.check_call([exe, tmp])
+    os.replace(tmp, MT_TABLE)
+    return MT_TABLE
 
 
 if __name__ == "__main__":

@@ -159,6 +159,31 @@ cudaError_t dev_alloc(void **p, size_t bytes, cudaStream_t stream)
 
 }  // namespace
 
+namespace {
+// the precomputed MT19937 polynomials, resident in device memory (one copy per device, uploaded
+// the first time a jump of a tabulated form needs them; 4.5 MB).  Record layout = MtOp (624 u32 words).
+const MtOp *mt_device_table(cudaStream_t stream)
+{
+    static std::mutex mu;
+    static const MtOp *per_device[64] = {};
+    const host::MtPoly *t = host::mt19937_table();
+    int dev = 0;
+    if (!t || cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!per_device[dev]) {
+        void *d = nullptr;
+        const size_t bytes = (size_t)host::MT_TABLE_ENTRIES * sizeof(MtOp);
+        static_assert(sizeof(MtOp) == sizeof(host::MtPoly), "table records are uploaded as they are");
+        if (cudaMalloc(&d, bytes) != cudaSuccess) return nullptr;
+        if (cudaMemcpyAsync(d, t, bytes, cudaMemcpyHostToDevice, stream) != cudaSuccess ||
+            cudaStreamSynchronize(stream) != cudaSuccess) { cudaFree(d); return nullptr; }
+        g_h2d_bytes.fetch_add(bytes, std::memory_order_relaxed);
+        per_device[dev] = (const MtOp *)d;
+    }
+    return per_device[dev];
+}
+}  // namespace
+
 struct prand_state {
     int gen;
     int device;
@@ -502,6 +527,28 @@ extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_l
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     st->last_stream = stream;
     Dist n = {steps_mant, steps_log2};
+    if (st->gen == PRAND_MT19937) {
+        // a tabulated distance is one application of a device-resident polynomial; any other
+        // distance "reduces to jumping ahead blocks of lengths 2^i1, ..., 2^il" of the binary notation, applied
+        // one after the other on the device -- no host polynomial arithmetic.  With many streams and many set
+        // bits the applications cost more than the host products that merge them (~1.5 ms each against ~1 us
+        // per stream and application): then the host multiplies the tabulated polynomials and one application runs.
+        std::vector<int> terms;
+        if (host::mt19937_table() && host::mt19937_table_terms(n, terms)) {
+            const double app_us = st->ns < 100 ? 90.0 : 0.9 * (double)st->ns;
+            const double device_us = terms.size() * app_us, host_us = (terms.size() - 1) * 1500.0 + app_us;
+            if (const MtOp *table = device_us <= host_us ? mt_device_table(stream) : nullptr) {
+                uint32_t *d = (uint32_t *)st->d_state[st->cur];
+                for (int t : terms) {
+                    LaunchInfo li;
+                    CU(mt19937_apply(stream, d, d, 0, st->ns, 0, table + t, &li));
+                    li.kernel = "mt19937_apply<table>";
+                    note(st, li);
+                }
+                return PRAND_OK;
+            }
+        }
+    }
     int rc = jump_prepare(st, n, stream);
     if (rc) return rc;
     rc = jump_launch(st, stream, &n);
@@ -1126,6 +1173,16 @@ extern "C" int prand_host_mt19937_mulmod(const uint32_t *a624, const uint32_t *b
     std::memcpy(b.w, b624, sizeof b.w);
     host::mt19937_mulmod(r, a, b);
     std::memcpy(r624, r.w, sizeof r.w);
+    return PRAND_OK;
+}
+
+extern "C" int prand_host_mt19937_table(uint64_t mant, unsigned log2, uint32_t *words624)
+{
+    if (!words624 || log2 > 32768) return PRAND_ERR_ARG;
+    const host::MtPoly *t = host::mt19937_table();
+    const int idx = t ? host::mt19937_table_index(Dist{mant, log2}) : -1;
+    if (idx < 0) return PRAND_ERR_ARG;
+    std::memcpy(words624, t[idx].w, sizeof t[idx].w);
     return PRAND_OK;
 }
 

@@ -1,8 +1,12 @@
 // skip_ops.cpp -- host-side preparation of the skip operators; see skip_ops.h.
 // Product code: shares nothing with oracle/.
 #include "skip_ops.h"
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
+#include <dlfcn.h>
 #include <mutex>
+#include <string>
 
 namespace prand {
 namespace host {
@@ -358,7 +362,88 @@ void mt19937_mulmod(MtPoly &r, const MtPoly &a, const MtPoly &b)
     std::memcpy(r.w, prod, sizeof r.w);
 }
 
+// ---- the precomputed table ------------------------------------------------------------
+namespace {
+std::vector<MtPoly> g_table;
+bool g_table_tried = false;
+std::mutex g_table_mu;
+
+std::string table_path()
+{
+    if (const char *env = std::getenv("PRAND_MT_TABLE")) return env;
+    Dl_info info;
+    if (dladdr((const void *)&mt19937_seed_state, &info) && info.dli_fname) {
+        std::string p = info.dli_fname;
+        const size_t slash = p.rfind('/');
+        return (slash == std::string::npos ? std::string(".") : p.substr(0, slash)) + "/mt19937_polys.bin";
+    }
+    return "mt19937_polys.bin";
+}
+}  // namespace
+
+const MtPoly *mt19937_table()
+{
+    if (prand::debug_hooks().mt_host_poly) return nullptr;     // hook: every polynomial by host arithmetic
+    std::lock_guard<std::mutex> lock(g_table_mu);
+    if (!g_table_tried) {
+        g_table_tried = true;
+        if (FILE *f = std::fopen(table_path().c_str(), "rb")) {
+            std::vector<MtPoly> t(MT_TABLE_ENTRIES);
+            const size_t n = std::fread(t.data(), sizeof(MtPoly), t.size(), f);
+            char extra;
+            const bool exact = n == t.size() && std::fread(&extra, 1, 1, f) == 0;
+            std::fclose(f);
+            // record 0 must be the polynomial x, record 1 x^2: a cheap guard against a foreign file
+            if (exact && t[0].w[0] == 2 && t[1].w[0] == 4) g_table.swap(t);
+        }
+    }
+    return g_table.empty() ? nullptr : g_table.data();
+}
+
+int mt19937_table_index(Dist v)
+{
+    if (v.mant == 0) return -1;
+    const unsigned tz = (unsigned)__builtin_ctzll(v.mant);
+    const uint64_t odd = v.mant >> tz;
+    const uint64_t log2 = (uint64_t)v.log2 + tz;
+    if (odd == 1) return log2 < (uint64_t)MT_TABLE_POW2 ? (int)log2 : -1;
+    // m 2^i with m in 15..24: m = odd 2^k for some k <= 4 taken from the power of two
+    for (unsigned k = 0; k <= 4 && k <= log2; k++) {
+        const uint64_t m = odd << k;
+        if (m > (uint64_t)MT_TABLE_M1) break;
+        if (m >= (uint64_t)MT_TABLE_M0 && log2 - k < (uint64_t)MT_TABLE_SHIFTS)
+            return MT_TABLE_POW2 + (int)(m - MT_TABLE_M0) * MT_TABLE_SHIFTS + (int)(log2 - k);
+    }
+    return -1;
+}
+
+bool mt19937_table_terms(Dist v, std::vector<int> &idx)
+{
+    idx.clear();
+    const int whole = mt19937_table_index(v);
+    if (whole >= 0) { idx.push_back(whole); return true; }
+    for (uint64_t e = v.mant; e; e &= e - 1) {
+        const uint64_t n = (uint64_t)__builtin_ctzll(e) + v.log2;
+        if (n >= (uint64_t)MT_TABLE_POW2) { idx.clear(); return false; }
+        idx.push_back((int)n);
+    }
+    return true;
+}
+
 void mt19937_xpow(Dist n, MtPoly &out)
+{
+    // tabulated distances cost a copy; sums of tabulated distances one product per extra term
+    std::vector<int> idx;
+    const MtPoly *t = mt19937_table();
+    if (t && n.mant && mt19937_table_terms(n, idx) && idx.size() <= 8) {
+        out = t[idx[0]];
+        for (size_t k = 1; k < idx.size(); k++) mt19937_mulmod(out, out, t[idx[k]]);
+        return;
+    }
+    mt19937_xpow_raw(n, out);
+}
+
+void mt19937_xpow_raw(Dist n, MtPoly &out)
 {
     MtPoly acc;
     std::memset(&acc, 0, sizeof acc);
@@ -401,9 +486,13 @@ void mt19937_levels(Dist n, unsigned levels, std::vector<MtPoly> &out)
         hit = cache.size() - 1;
     }
     std::vector<MtPoly> &lad = cache[hit].ladder;
+    const MtPoly *table = mt19937_table();
     while (lad.size() < levels) {
         lad.emplace_back();
-        mt19937_sqrmod(lad[lad.size() - 1], lad[lad.size() - 2]);
+        const Dist d = {n.mant, n.log2 + (unsigned)(lad.size() - 1)};
+        const int ti = table && n.mant ? mt19937_table_index(d) : -1;
+        if (ti >= 0) lad.back() = table[ti];
+        else mt19937_sqrmod(lad[lad.size() - 1], lad[lad.size() - 2]);
     }
     for (unsigned lev = 0; lev < levels; lev++) out[lev] = lad[lev];
 }

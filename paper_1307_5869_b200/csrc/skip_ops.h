@@ -41,7 +41,18 @@ struct MtPoly { uint64_t w[MT_PW]; };              // bit (i & 63) of w[i >> 6] 
 const MtPoly &mt19937_phi();                       // characteristic polynomial (closed form of ref. [2])
 void mt19937_mulmod(MtPoly &r, const MtPoly &a, const MtPoly &b);   // r = a b mod phi
 void mt19937_sqrmod(MtPoly &r, const MtPoly &a);                     // r = a^2 mod phi
-void mt19937_xpow(Dist n, MtPoly &out);                              // x^n mod phi
+void mt19937_xpow(Dist n, MtPoly &out);                              // x^n mod phi (table entries where they apply)
+void mt19937_xpow_raw(Dist n, MtPoly &out);                          // x^n mod phi by square-and-multiply only
+
+// The precomputed table of: x^v mod phi for v = 2^n (n < 512) and v = m 2^i (m = 15..24, i < 128),
+// written by csrc/mt_table_gen.cpp at build time and loaded from the file next to the library.
+constexpr int MT_TABLE_POW2 = 512, MT_TABLE_M0 = 15, MT_TABLE_M1 = 24, MT_TABLE_SHIFTS = 128;
+constexpr int MT_TABLE_ENTRIES = MT_TABLE_POW2 + (MT_TABLE_M1 - MT_TABLE_M0 + 1) * MT_TABLE_SHIFTS;   // 1792
+const MtPoly *mt19937_table();                    // MT_TABLE_ENTRIES records, or nullptr (no file / hook PRAND_MT_POLY=host)
+int mt19937_table_index(Dist v);                  // record of x^v, or -1 if v is not of a tabulated form
+// v as a sum of tabulated distances (binary decomposition of the mantissa): record indices in
+// `idx`; false if some term is not tabulated (2^n with n >= 512)
+bool mt19937_table_terms(Dist v, std::vector<int> &idx);
 void mt19937_levels(Dist n, unsigned levels, std::vector<MtPoly> &out);
 void mt19937_to_op(const MtPoly &p, MtOp &op);                       // repack as 32-bit words
 void mt19937_seed_state(uint32_t seed, uint32_t *w624);              // ref.-[2] initialiser

@@ -286,6 +286,33 @@ def test_device_callable_api_matches_oracle_and_bulk_kernels(gen):
         assert st == wst
 
 
+def test_mt19937_jumps_use_the_precomputed_polynomial_table():
+    """tabulated distances (2^n, n < 512; m 2^i, m = 15..24, i < 128) are one application of a
+    device-resident polynomial; other distances are applied term by term of their binary notation; distances
+    outside the table, or everything under PRAND_MT_POLY=host, go through the host's polynomial arithmetic.
+    All must reach the oracle's state."""
+    need_gpu()
+    cases = [(2**20, "mt19937_apply<table>"), (20 << 30, "mt19937_apply<table>"), (5, "mt19937_apply<table>"),
+             (12345, "mt19937_apply<table>"), (3 << 500, "mt19937_apply<table>"), (1 << 600, "mt19937_apply"),
+             ((2**40 + 1) << 480, "mt19937_apply")]
+    for steps, kernel in cases:
+        w = Workload("mt-table", "mt19937", 5489, 3, 2**64, 30, "u32")
+        want, wst = oracle_run(w, pre_jump=steps)
+        for host in (False, True):
+            P.prand_debug_set("PRAND_MT_POLY", "host" if host else None)
+            try:
+                g = P.Generator("mt19937", 5489, 3, 2**64)
+                g.jump(steps)
+                assert g.last_kernel == ("mt19937_apply" if host else kernel), (steps, g.last_kernel)
+                got = g.generate(30, "u32").cpu().numpy().view(np.uint32)
+                st = g.state()
+                g.close()
+            finally:
+                P.prand_debug_set("PRAND_MT_POLY", None)
+            assert_same(w, got, want)
+            assert st == wst
+
+
 def test_lfsr113_table_method_equals_matrix_jumps_and_oracle():
     """PAPER.md:363-370 (section 5.3): the paper's own jump algorithm for LFSR113 -- 128 tables per stream
     built by eq. 9, one warp per stream -- as an alternate of the GF(2) matrix path (PRAND_LFSR_INIT=table):

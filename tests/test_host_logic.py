@@ -143,6 +143,32 @@ def test_mt19937_polynomial_product_composes_jumps():
         assert np.array_equal(prod, oracle.mt19937_jump_poly(a + b))
 
 
+def test_mt19937_precomputed_table_is_the_papers_and_equals_the_oracle():
+    """x^v mod phi stored for v = 2^n (n = 0..511) and v = m 2^i (m = 15..24, i = 0..127),
+    2496 bytes each, < 5 MB.  Every record is pinned: the first of each chain (x, x^15 .. x^24) and deep
+    ones against the oracle's own square-and-multiply, every other record as the square of its predecessor
+    by the polynomial product (itself pinned to the oracle above)."""
+    entries = [(1, n) for n in range(512)] + [(m, i) for m in range(15, 25) for i in range(128)]
+    assert len(entries) == 1792 and len(entries) * 2496 < 5 * 2**20
+    recs = {}
+    for m, i in entries:
+        r = P.prand_host_mt19937_table(m << i)
+        assert r is not None, (m, i)
+        recs[(m, i)] = r
+    # not tabulated: other odd parts, powers beyond the table
+    for v in (3, 7 << 10, 25 << 127, 2**512, 13 << 3, 15 << 128):
+        assert P.prand_host_mt19937_table(v) is None
+    # 16 = 2^4, 20 2^i = 5 2^(i+2) ...: one distance, one polynomial, whichever chain names it
+    assert recs[(16, 3)] == recs[(1, 7)] and recs[(24, 0)] == P.prand_host_mt19937_table(3 << 3)
+    # anchors against the oracle
+    for m, i in [(1, 0), (1, 1), (1, 64), (1, 511)] + [(m, 0) for m in range(15, 25)] + [(15, 64), (24, 127)]:
+        assert np.array_equal(np.frombuffer(recs[(m, i)], dtype=np.uint64), oracle.mt19937_jump_poly(m << i)), (m, i)
+    # every record is the square of its predecessor
+    for m, i in entries:
+        if i:
+            assert P.prand_host_mt19937_mulmod(recs[(m, i - 1)], recs[(m, i - 1)]) == recs[(m, i)], (m, i)
+
+
 def test_mt19937_seed_state_equals_oracle():
     mine = np.frombuffer(P.prand_host_seed_state("mt19937", 5489), dtype=np.uint32).copy()
     want = np.frombuffer(oracle.State("mt19937", 5489).export(), dtype=np.uint32)
