@@ -323,6 +323,46 @@ def time_config(torch, P, w, steps, warmup, flush, peak, peak_src, device_index=
             "clocks": clk.summary()}
 
 
+def jump_methods(torch, P):
+    """the paper's own jump algorithms beside the library's default ones -- best wall time of
+    prand_init + synchronise (3 runs) for 2^20 LFSR113 streams by the GF(2) matrix path and by the 128-table
+    method, and of a prand_jump of 2^20 MT19937 steps on 512 streams from the device-resident
+    polynomial table against host polynomial arithmetic with a cold cache."""
+    def best(fn, reps=3):
+        ts = []
+        for _ in range(reps):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            fn()
+            torch.cuda.synchronize()
+            ts.append((time.perf_counter() - t0) * 1e3)
+        return min(ts)
+
+    out = {}
+    w = workloads.ALL["C5-lfsr113"]
+    for name, hook in (("matrix", None), ("table", "table")):
+        P.prand_debug_set("PRAND_LFSR_INIT", hook)
+        hs = []
+        out[f"lfsr113_init_{w.n_streams}_streams_{name}_ms"] = best(
+            lambda: hs.append(P.prand_init(w.gen, w.seed, w.n_streams, w.block_len)))
+        for h in hs:
+            P.prand_free(h)
+    P.prand_debug_set("PRAND_LFSR_INIT", None)
+    c3 = workloads.ALL["C3"]
+    h = P.prand_init(c3.gen, c3.seed, c3.n_streams, c3.block_len)
+    k = [0]
+
+    def jump():
+        k[0] += 1
+        P.prand_jump(h, 1 << (20 + k[0]))             # a new tabulated distance every time: no cached ladder helps
+    out["mt19937_jump_512_streams_table_ms"] = best(jump)
+    P.prand_debug_set("PRAND_MT_POLY", "host")
+    out["mt19937_jump_512_streams_host_polynomial_ms"] = best(jump)
+    P.prand_debug_set("PRAND_MT_POLY", None)
+    P.prand_free(h)
+    return out
+
+
 def run_ours(args, w):
     import torch
     import paper_1307_5869_b200 as P
@@ -459,6 +499,7 @@ def run_ours(args, w):
                                     local_rank))
             print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
         line["per_config"] = rows
+        line["jump_methods"] = jump_methods(torch, P)
         line["per_config_note"] = ("generation call alone (prand_generate_* / prand_generate_seq_*), CUDA-event median of "
                                    f"{args.config_steps} calls after 3 warm-ups, 256 MB written before each call (L2 flush); "
                                    "frac: hbm = algorithmic bytes (output + 2 x state) / gen_ms / MEASURED_PEAKS hbm_gbs; "

@@ -63,7 +63,7 @@ enum prand_error {
     PRAND_ERR_CUDA = -5,       /* a CUDA runtime call failed; prand_last_cuda_error() has it  */
     PRAND_ERR_SIZE = -6,       /* byte count does not match prand_state_bytes()               */
     PRAND_ERR_ALLOC = -7,      /* host or device allocation failed                            */
-    PRAND_ERR_INTERNAL = -8    /* self-check of a prepared operator failed                    */
+    PRAND_ERR_INTERNAL = -8    /* MT19937: the characteristic polynomial failed its self-check  */
 };
 
 /*
@@ -203,6 +203,9 @@ int prand_device_api_fill_f64(prand_state *st, double *out, uint64_t n_per_strea
  *   MT19937   624 x u32 window x_P..x_{P+623}, low 31 bits of word 0 zeroed;
  *   GM/GQ     2s words xP_0, xN_0, ..., xP_{s-1}, xN_{s-1} (u32 if g < 2^32, else u64), residues mod g.
  * prand_state_bytes() = n_streams * per-stream bytes.  Both calls synchronise the device.
+ * prand_set_state checks the words: LFSR113 components with all significant bits zero, MRG32K3A words that are
+ * not residues mod m1 / m2 or a component that is all zero, and GM/GQ words >= g are refused (PRAND_ERR_ARG,
+ * nothing is changed).
  */
 size_t prand_state_bytes(const prand_state *st);
 int prand_get_state(const prand_state *st, void *host_buf, size_t bytes);
@@ -211,8 +214,24 @@ int prand_set_state(prand_state *st, const void *host_buf, size_t bytes);
 uint64_t prand_n_streams(const prand_state *st);
 int prand_gen_of(const prand_state *st);
 
-/* Releases the state and every device buffer it owns (synchronises the device first). */
+/*
+ * Releases the state and every device buffer it owns.  The release is STREAM-ORDERED on the CUDA stream of
+ * the state's most recent call (no device synchronisation): work queued there before prand_free still sees
+ * the buffers; the caller must not have work on OTHER streams that still uses the state or the pointer of
+ * prand_state_device_ptr / prand_device_ops.
+ */
 int prand_free(prand_state *st);
+
+/*
+ * Device memory comes from a stream-ordered pool owned by the library (one per device, never shrunk, so that
+ * prand_init + prand_free cost microseconds).  prand_trim returns the pool's unused memory of the current
+ * device to the driver; call it after freeing large states if other allocators need the memory.
+ */
+int prand_trim(void);
+
+/* MT19937: the generation kernels address a row block with 32-bit byte offsets; prand_init refuses more streams
+ * per state (PRAND_ERR_ARG).  2.58 million streams = 6.4 GB of state; shard larger families (prand_init_shard). */
+#define PRAND_MT19937_MAX_STREAMS 2581102ull
 
 /*
  * prand_fill_u32 -- write-peak probe: 128-bit stores of a constant to `n_words` u32 at device

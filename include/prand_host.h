@@ -33,6 +33,10 @@ int prand_host_seed_state(int gen, uint64_t seed, void *buf, size_t bytes);
 /* MT19937 characteristic polynomial phi, 624 u32 words, bit 19937 is the leading coefficient. */
 int prand_host_mt19937_phi(uint32_t *words624);
 
+/* The check prand_init makes once per process before it accepts MT19937: phi(A) annihilates a window of the
+ * recurrence (Cayley-Hamilton).  0, or PRAND_ERR_INTERNAL. */
+int prand_host_mt19937_phi_selfcheck(void);
+
 /* r = a b mod phi on 624-word coefficient arrays (the product used to combine level polynomials). */
 int prand_host_mt19937_mulmod(const uint32_t *a624, const uint32_t *b624, uint32_t *r624);
 

@@ -60,6 +60,7 @@ _SIGS = {
     "prand_probe_pipe_name": (C.c_char_p, [C.c_int]),
     "prand_probe_pipe": (C.c_int, [C.c_int, C.c_uint64, C.POINTER(C.c_uint64), C.c_void_p]),
     "prand_debug_set": (C.c_int, [C.c_char_p, C.c_char_p]),
+    "prand_trim": (C.c_int, []),
     "prand_launch_count": (C.c_uint64, []),
     "prand_uploaded_bytes": (C.c_uint64, []),
     "prand_last_kernel": (C.c_char_p, [C.c_void_p]),
@@ -72,6 +73,7 @@ _SIGS = {
     "prand_host_state_bytes": (C.c_size_t, [C.c_int]),
     "prand_host_seed_state": (C.c_int, [C.c_int, C.c_uint64, C.c_void_p, C.c_size_t]),
     "prand_host_mt19937_phi": (C.c_int, [C.c_void_p]),
+    "prand_host_mt19937_phi_selfcheck": (C.c_int, []),
     "prand_host_mt19937_mulmod": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p]),
     "prand_host_mt19937_table": (C.c_int, [C.c_uint64, C.c_uint, C.c_void_p]),
     "prand_host_gm_kq": (C.c_int, [C.c_int, C.c_uint64, C.c_uint, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),

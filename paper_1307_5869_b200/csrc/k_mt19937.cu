@@ -308,12 +308,9 @@ template <int S, int T, int M, int DT, int HI, bool PAIR> cudaError_t launch_gen
     typedef typename OutElem<DT>::type E;
     auto kern = mt19937_gen_kernel<S, T, M, DT, HI, PAIR>;
     const size_t smem = (size_t)2 * S * MtPitch<S>::value * sizeof(uint32_t);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // per launch, not once per process: the attribute belongs to the current device's context
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     uint64_t blocks = ceil_div_u64(a.n_streams, S);
     if (PAIR) blocks += blocks & 1;
     cudaLaunchConfig_t cfg = {};
@@ -504,12 +501,8 @@ template <int DT, int HI> cudaError_t launch_bgen(cudaStream_t stream, const Gen
     typedef typename OutElem<DT>::type E;
     auto kern = mt19937_bgen_kernel<DT, HI>;
     const size_t smem = (size_t)32 * BP * sizeof(uint32_t);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   // per device
+    if (e != cudaSuccess) return e;
     const uint64_t blocks = ceil_div_u64(a.n_streams, 32);
     const MtMul c = {2u * 0x1908B0DFu, 1u << 31, 1u << 21, 1u << 14};
     kern<<<(unsigned)blocks, BW * 32, smem, stream>>>((const uint32_t *)a.st_in, (uint32_t *)a.st_out, (E *)a.out,
@@ -995,22 +988,16 @@ template <int DT> cudaError_t launch_cgen(cudaStream_t stream, const GenArgs &a)
 cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
                           uint64_t count, uint64_t src_back, const MtOp *d_op, LaunchInfo *li)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(mt19937_apply_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)APPLY_SMEM);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(mt19937_apply_kernel<640, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)APPLY_SMEM);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(mt19937_apply_kernel<160, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)APPLY_SMEM);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(mt19937_apply_win_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)APPLY_SMEM);
-        if (e != cudaSuccess) return e;
-        attr_set = true;
-    }
+    // the opt-in belongs to the current device's context: set it per call (a microsecond), not once per process
+    cudaError_t e = cudaFuncSetAttribute(mt19937_apply_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)APPLY_SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(mt19937_apply_kernel<640, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)APPLY_SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(mt19937_apply_kernel<160, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)APPLY_SMEM);
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(mt19937_apply_win_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)APPLY_SMEM);
+    if (e != cudaSuccess) return e;
     li->kernel = "mt19937_apply";
     li->launches = 0;
     // grid.x is limited to 2^31-1 blocks; streams beyond that would not fit device memory anyway
@@ -1043,8 +1030,9 @@ cudaError_t mt19937_seq(cudaStream_t stream, const void *st_in, void *st_last, v
 cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *li)
 {
     li->launches = 1;
-    // a thread's byte offset inside a row block must fit 32 bits (wave of 208 rows, 8-byte elements)
-    if (a.n_streams > ((1ull << 32) / (208 * 8)) - 8) return cudaErrorInvalidValue;
+    // a thread's byte offset inside a row block must fit 32 bits (wave of 208 rows, 8-byte elements);
+    // prand_init refuses larger families (PRAND_MT19937_MAX_STREAMS, prand.h)
+    if (a.n_streams > PRAND_MT19937_MAX_STREAMS) return cudaErrorInvalidValue;
     // Kernel choice by stream count (measured on B200): 32 streams per CTA need >= ~128
     // CTAs; below that 8 streams per CTA; below ~1000 streams 4 per CTA in sector-sharing cluster pairs.
     int cfg = a.n_streams >= 4096 ? 0 : a.n_streams >= 1024 ? 1 : 2;

@@ -133,28 +133,42 @@ int cuda_fail(cudaError_t e)
         if (e_ != cudaSuccess) return cuda_fail(e_);     \
     } while (0)
 
-// Device memory comes from the stream-ordered allocator (cudaMallocAsync on the default pool, kept
-// warm by a release threshold of "never"): init / free of a state cost microseconds and never
-// synchronise the device, so that prand_init + prand_generate + prand_free can be a hot loop.
-cudaError_t pool_setup()
+// Device memory comes from the stream-ordered allocator, from a pool of the library's own (one per device,
+// release threshold "never": init / free of a state cost microseconds and never synchronise the device, so
+// that prand_init + prand_generate + prand_free can be a hot loop).  The process's default pool is left
+// alone; prand_trim() hands the cached memory back to the driver.
+std::mutex g_pool_mu;
+cudaMemPool_t g_pools[64] = {};
+cudaError_t device_pool(cudaMemPool_t *pool)
 {
-    static cudaError_t status = [] {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e != cudaSuccess) return e;
-        cudaMemPool_t pool;
-        e = cudaDeviceGetDefaultMemPool(&pool, dev);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (!g_pools[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t p;
+        e = cudaMemPoolCreate(&p, &props);
         if (e != cudaSuccess) return e;
         uint64_t keep = UINT64_MAX;
-        return cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-    }();
-    return status;
+        e = cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) { cudaMemPoolDestroy(p); return e; }
+        g_pools[dev] = p;
+    }
+    *pool = g_pools[dev];
+    return cudaSuccess;
 }
 cudaError_t dev_alloc(void **p, size_t bytes, cudaStream_t stream)
 {
-    cudaError_t e = pool_setup();
+    cudaMemPool_t pool;
+    cudaError_t e = device_pool(&pool);
     if (e != cudaSuccess) return e;
-    return cudaMallocAsync(p, bytes ? bytes : 1, stream);
+    return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, stream);
 }
 
 }  // namespace
@@ -441,6 +455,8 @@ extern "C" int prand_init_shard(prand_state **out, int gen, uint64_t seed, uint6
     if (block_len_mant == 0 && block_len_log2 != 0) return PRAND_ERR_ARG;
     if (block_len_log2 > 4096) return PRAND_ERR_ARG;
     if (first_stream + n_streams < first_stream) return PRAND_ERR_OVERFLOW;
+    if (gen == PRAND_MT19937 && n_streams > PRAND_MT19937_MAX_STREAMS) return PRAND_ERR_ARG;
+    if (gen == PRAND_MT19937 && !host::mt19937_phi_selfcheck()) return PRAND_ERR_INTERNAL;
     {
         unsigned __int128 top = (unsigned __int128)(first_stream + n_streams - 1) * block_len_mant;
         if (top >> 64) return PRAND_ERR_OVERFLOW;
@@ -607,13 +623,29 @@ void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t 
 int ensure_chunk_ops(prand_state *st, uint64_t chunk_len, uint64_t n_chunks, cudaStream_t stream)
 {
     if (st->d_chunk_ops && st->chunk_len == chunk_len && st->chunk_count >= n_chunks) return PRAND_OK;
-    // operator of distance c * chunk_len for c = 1..n_chunks-1: one application per virtual stream
-    std::vector<unsigned char> ops, one;
-    for (uint64_t c = 1; c < n_chunks; c++) {
-        Dist d = {c * chunk_len, 0};
-        int rc = build_level_ops(st->gen, d, 1, one);
-        if (rc) return rc;
-        ops.insert(ops.end(), one.begin(), one.end());
+    // operator of distance c * chunk_len for c = 1..n_chunks-1: one application per virtual stream.  The host
+    // bytes of the most recent (generator, chunk_len, n_chunks) plans are kept for the process, so that a state
+    // created per step (init + generate + free) does not pay the preparation again.
+    struct Plan { int gen; uint64_t len, n; std::vector<unsigned char> bytes; };
+    static std::mutex mu;
+    static std::vector<Plan> plans;                        // most recent last, at most 8
+    std::vector<unsigned char> ops;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        for (const Plan &p : plans)
+            if (p.gen == st->gen && p.len == chunk_len && p.n == n_chunks) ops = p.bytes;
+    }
+    if (ops.empty()) {
+        std::vector<unsigned char> one;
+        for (uint64_t c = 1; c < n_chunks; c++) {
+            Dist d = {c * chunk_len, 0};
+            int rc = build_level_ops(st->gen, d, 1, one);
+            if (rc) return rc;
+            ops.insert(ops.end(), one.begin(), one.end());
+        }
+        std::lock_guard<std::mutex> lock(mu);
+        if (plans.size() == 8) plans.erase(plans.begin());
+        plans.push_back(Plan{st->gen, chunk_len, n_chunks, ops});
     }
     if (st->d_chunk_ops) { CU(cudaFreeAsync(st->d_chunk_ops, stream)); st->d_chunk_ops = nullptr; }
     CU(dev_alloc(&st->d_chunk_ops, ops.size(), stream));
@@ -1045,6 +1077,30 @@ extern "C" int prand_set_state(prand_state *st, const void *host_buf, size_t byt
         CU(cudaMemcpy(st->d_state[st->cur], host_buf, bytes, cudaMemcpyHostToDevice));
         return PRAND_OK;
     }
+    // the kernels' exactness arguments assume canonical residues and live (non-degenerate) components
+    if (st->gen == PRAND_LFSR113) {
+        static const uint32_t top[4] = {0xFFFFFFFEu, 0xFFFFFFF8u, 0xFFFFFFF0u, 0xFFFFFF80u};
+        const uint32_t *w = (const uint32_t *)host_buf;
+        for (uint64_t i = 0; i < st->ns * 4; i++)
+            if ((w[i] & top[i & 3]) == 0) return PRAND_ERR_ARG;                 // a component stuck at zero
+    } else if (st->gen == PRAND_MRG32K3A) {
+        const uint32_t *w = (const uint32_t *)host_buf;
+        for (uint64_t s = 0; s < st->ns; s++, w += 6) {
+            for (int k = 0; k < 6; k++)
+                if (w[k] >= (k < 3 ? 4294967087u : 4294944443u)) return PRAND_ERR_ARG;   // not a residue mod m1 / m2
+            if ((w[0] | w[1] | w[2]) == 0 || (w[3] | w[4] | w[5]) == 0) return PRAND_ERR_ARG;
+        }
+    } else if (const GmParams *gp = gm_params(st->gen)) {
+        if (gp->wide) {
+            const uint64_t *w = (const uint64_t *)host_buf;
+            for (size_t i = 0; i < st->ns * words; i++)
+                if (w[i] >= gp->g) return PRAND_ERR_ARG;
+        } else {
+            const uint32_t *w = (const uint32_t *)host_buf;
+            for (size_t i = 0; i < st->ns * words; i++)
+                if (w[i] >= gp->g) return PRAND_ERR_ARG;
+        }
+    }
     std::vector<unsigned char> tmp(bytes);
     if (const GmParams *gp = gm_params(st->gen)) {
         // GM55/GQ58 (g = 2^t p): the fast kernels need every word to be a multiple of 2^t
@@ -1080,6 +1136,15 @@ extern "C" int prand_fill_u32(uint32_t *out, uint64_t n_words, uint32_t value, v
     LaunchInfo li = {"", 0};
     CU(fill_u32((cudaStream_t)cuda_stream, out, n_words, value, &li));
     note(nullptr, li);
+    return PRAND_OK;
+}
+
+extern "C" int prand_trim(void)
+{
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (dev >= 0 && dev < 64 && g_pools[dev]) CU(cudaMemPoolTrimTo(g_pools[dev], 0));
     return PRAND_OK;
 }
 
@@ -1163,6 +1228,11 @@ extern "C" int prand_host_mt19937_phi(uint32_t *words624)
     host::mt19937_to_op(host::mt19937_phi(), op);
     std::memcpy(words624, op.w, sizeof op.w);
     return PRAND_OK;
+}
+
+extern "C" int prand_host_mt19937_phi_selfcheck(void)
+{
+    return host::mt19937_phi_selfcheck() ? PRAND_OK : PRAND_ERR_INTERNAL;
 }
 
 extern "C" int prand_host_mt19937_mulmod(const uint32_t *a624, const uint32_t *b624, uint32_t *r624)

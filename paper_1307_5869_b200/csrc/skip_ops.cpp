@@ -227,7 +227,7 @@ bool gm_seed_state(const GmParams &p, uint64_t seed, uint64_t *words)
 // form (ref. [2], appendix; w - r = 1 here)
 //     phi(t) = u (v^31 + a_0 v^30 + ... + a_29 v + a_30) + a_31,   u = t^n + t^m, v = t^(n-1) + t^(m-1),
 // a_i = bit i of a (a_31 is the most significant bit).  It is evaluated by Horner's rule in v with
-// shift-and-xor products; prand_init self-checks it (phi(A) applied to a window must vanish).
+// shift-and-xor products; prand_init self-checks it once per process (mt19937_phi_selfcheck below).
 // ==================================================================================================
 namespace {
 constexpr int WIDE = 2 * MT_PW;                      // words of an unreduced product
@@ -314,6 +314,30 @@ inline uint64_t spread32(uint32_t x)                  // bit i -> bit 2i
 }  // namespace
 
 const MtPoly &mt19937_phi() { return phi_data().phi; }
+
+// phi(A) W = 0 (Cayley-Hamilton): sum over the set coefficients i of x_{i+j} must vanish for every word j >= 1 of
+// a window and for the top bit of word 0.  Checked once per process on the sequence of seed 1; prand_init
+// refuses MT19937 (PRAND_ERR_INTERNAL) if the closed form ever disagreed with the recurrence.
+bool mt19937_phi_selfcheck()
+{
+    static const bool ok = [] {
+        const PhiData &d = phi_data();
+        std::vector<uint32_t> x(MT_DEG + MT_N + 1);
+        mt19937_seed_state(1u, x.data());
+        for (int k = 0; k + MT_N < (int)x.size(); k++) {
+            const uint32_t y = (x[k] & 0x80000000u) | (x[k + 1] & 0x7FFFFFFFu);
+            x[k + MT_N] = x[k + MT_M] ^ (y >> 1) ^ ((y & 1u) ? 0x9908B0DFu : 0u);
+        }
+        for (int j = 0; j < 4; j++) {
+            uint32_t acc = x[MT_DEG + j];                  // leading coefficient
+            for (int e : d.low_terms) acc ^= x[e + j];
+            if (j == 0) acc &= 0x80000000u;                // only the top bit of word 0 is state
+            if (acc) return false;
+        }
+        return true;
+    }();
+    return ok;
+}
 
 void mt19937_sqrmod(MtPoly &r, const MtPoly &a)
 {

@@ -39,6 +39,7 @@ constexpr int MT_N = 624, MT_M = 397, MT_DEG = 19937;
 constexpr int MT_PW = 312;                         // 64-bit words of a polynomial of degree < 19968
 struct MtPoly { uint64_t w[MT_PW]; };              // bit (i & 63) of w[i >> 6] = coefficient of x^i
 const MtPoly &mt19937_phi();                       // characteristic polynomial (closed form of ref. [2])
+bool mt19937_phi_selfcheck();                      // phi(A) annihilates a generated window (checked once per process)
 void mt19937_mulmod(MtPoly &r, const MtPoly &a, const MtPoly &b);   // r = a b mod phi
 void mt19937_sqrmod(MtPoly &r, const MtPoly &a);                     // r = a^2 mod phi
 void mt19937_xpow(Dist n, MtPoly &out);                              // x^n mod phi (table entries where they apply)

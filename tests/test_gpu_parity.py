@@ -286,6 +286,38 @@ def test_device_callable_api_matches_oracle_and_bulk_kernels(gen):
         assert st == wst
 
 
+def test_set_state_refuses_words_the_kernels_cannot_take():
+    """The hot loops assume canonical residues and live components (x < m1, y < m2, GM words < g, no LFSR113
+    component stuck at zero): prand_set_state range-checks an imported state and changes nothing on failure."""
+    need_gpu()
+    def try_set(gen, mutate, dt):
+        g = P.Generator(gen, workloads.SEED.get(gen, 1), 3, 1000)
+        good = g.state()
+        a = np.frombuffer(good, dtype=dt).copy()
+        mutate(a)
+        rc = P.lib().prand_set_state(g._h, a.tobytes(), len(good))
+        assert g.state() == (good if rc else a.tobytes())
+        g.close()
+        return rc
+    def put(i, v):
+        def f(a):
+            a[i] = v
+        return f
+    def zero(lo, hi):
+        def f(a):
+            a[lo:hi] = 0
+        return f
+    assert try_set("mrg32k3a", put(7, 2**32 - 209), np.uint32) == -2            # x word = m1
+    assert try_set("mrg32k3a", put(4, 2**32 - 22853), np.uint32) == -2          # y word = m2
+    assert try_set("mrg32k3a", zero(6, 9), np.uint32) == -2                     # x component all zero
+    assert try_set("lfsr113", put(5, 7), np.uint32) == -2                       # component 2: top 29 bits zero
+    assert try_set("gm31", put(3, 2**31 - 1), np.uint32) == -2                  # = g
+    assert try_set("gm61", put(10, 2**61 - 1), np.uint64) == -2
+    assert try_set("gq58.3", put(2, 2**29 * (2**29 - 3)), np.uint64) == -2
+    assert try_set("mrg32k3a", put(7, 2**32 - 210), np.uint32) == 0             # m1 - 1 is a residue
+    assert P.lib().prand_trim() == 0
+
+
 def test_mt19937_jumps_use_the_precomputed_polynomial_table():
     """tabulated distances (2^n, n < 512; m 2^i, m = 15..24, i < 128) are one application of a
     device-resident polynomial; other distances are applied term by term of their binary notation; distances

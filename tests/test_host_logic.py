@@ -67,6 +67,7 @@ def test_argument_errors_before_any_cuda_call():
     assert L.prand_init(C.byref(h), 2, 2**32, 4, 1, 0, None) == -3        # MT19937 seed >= 2^32
     assert L.prand_init(C.byref(h), 3, 2**19 - 1, 4, 1, 0, None) == -3    # GM19 seed = 0 mod g
     assert L.prand_init(C.byref(h), 0, 12345, 2**40, 2**40, 0, None) == -4  # s * mant overflows
+    assert L.prand_init(C.byref(h), 2, 5489, 2581103, 1, 64, None) == -2   # MT19937: more than PRAND_MT19937_MAX_STREAMS
     assert L.prand_init(None, 0, 12345, 4, 1, 0, None) == -2
     assert h.value is None
     assert L.prand_generate_u32(None, None, 4, None) == -2
@@ -126,6 +127,7 @@ def test_mt19937_phi_closed_form_equals_oracle_minimal_polynomial():
     assert deg == 19937
     assert np.array_equal(mine[:312], phi)
     assert sum(bin(int(w)).count("1") for w in mine) == 135     # 135 non-zero terms
+    assert P.lib().prand_host_mt19937_phi_selfcheck() == 0      # what prand_init checks once per process
 
 
 @pytest.mark.parametrize("dist", [0, 1, 5, 623, 624, 19937, 50000, 2**64, (2**40 + 5) << 64, 12345 << 3])
