@@ -139,3 +139,14 @@ def test_streams_threads_and_offsets_agree():
     part, st_part = oracle.streams("lfsr113", 12345, 5, 7, 1 << 40, 20, threads=3)
     assert np.array_equal(full[:, 5:], part)
     assert np.array_equal(st_full[5:], st_part)
+
+
+def test_survey_sample_values():
+    """tests/golden/survey_8c_samples.txt: the first five outputs for seed 12345 x 4 from the
+    surveyor's independent bit-level implementation of eqs. 7-8 (readings L1, L2: the seed's low bits are
+    ignored, the first output is the first stepped word)."""
+    import os
+    lines = [l for l in open(os.path.join(os.path.dirname(__file__), "golden", "survey_8c_samples.txt")) if not l.startswith("#")]
+    vals = {l.split(":")[0]: l.split(":")[1].split() for l in lines}
+    got = oracle.State("lfsr113", 12345).fill(5, "u32")
+    assert [int(v) for v in got] == [int(v) for v in vals["lfsr113 seed=12345 u32"]]

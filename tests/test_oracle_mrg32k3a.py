@@ -171,3 +171,20 @@ def test_block_splitting_is_positional():
     full, st_full = oracle.streams("mrg32k3a", 12345, 0, 10, 1 << 76, 12, "f64")
     part, st_part = oracle.streams("mrg32k3a", 12345, 4, 6, 1 << 76, 12, "f64", threads=2)
     assert np.array_equal(full[:, 4:], part) and np.array_equal(st_full[4:], st_part)
+
+
+def test_survey_sample_values_pin_the_combination_sign():
+    """tests/golden/survey_8c_samples.txt: the first outputs for seed 12345 x 6 from an
+    independent implementation.  They fix reading M1 -- z = (x - y) mod m1, not (x + y) -- and the
+    normalisation M3 (PAPER.md:347 is garbled on both)."""
+    import os
+    lines = [l for l in open(os.path.join(os.path.dirname(__file__), "golden", "survey_8c_samples.txt")) if not l.startswith("#")]
+    vals = {l.split(":")[0]: l.split(":")[1].split() for l in lines}
+    st = oracle.State("mrg32k3a", 12345)
+    z = st.fill(5, "u32")
+    assert [int(v) for v in z] == [int(v) for v in vals["mrg32k3a seed=12345 u32"]]
+    x, y, z0 = (int(v) for v in vals["mrg32k3a seed=12345 first_x_y_z"])
+    one = np.frombuffer(oracle.State("mrg32k3a", 12345).jump(1).export(), dtype=np.uint32)
+    assert (int(one[0]), int(one[3])) == (x, y) and (x - y) % (2**32 - 209) == z0 and (x + y) % (2**32 - 209) != z0
+    f = oracle.State("mrg32k3a", 12345).fill(1, "f64")[0]
+    assert f"{f:.16f}" == vals["mrg32k3a seed=12345 f64_first"][0] and f == z0 / (2**32 - 208)
