@@ -77,8 +77,9 @@ cudaError_t gm_tree_fill(cudaStream_t, int gen, void *st, uint64_t ns, uint64_t 
                          uint64_t back, uint64_t kn, uint64_t qn, LaunchInfo *);
 // MT19937: dst stream j (j in [dst0, dst0+count)) = g(A) applied to src stream (j - src_back), or to
 // itself when src_back == 0.  State layout [stream][624].
+// h_op: the same polynomial in host memory if the caller has it (it then travels as a kernel argument), else nullptr
 cudaError_t mt19937_apply(cudaStream_t, const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
-                          uint64_t count, uint64_t src_back, const MtOp *d_op, LaunchInfo *);
+                          uint64_t count, uint64_t src_back, const MtOp *d_op, const MtOp *h_op, LaunchInfo *);
 cudaError_t mt19937_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
 // sections of one sequence in PRAND's contiguous layout out[c * sec_len + i] (sec_len even, out 16-byte aligned);
 // st_in = [n_sections][624] windows, st_last (one window) receives the state after `length` numbers
@@ -104,7 +105,8 @@ int sm_count();   // multiprocessor count of the current device
 // launch paths read plain fields, never the environment.
 struct DebugHooks {
     int mt_cfg;             // PRAND_MT_CFG: force an MT19937 generation kernel variant (-1: by stream count)
-    bool mt_apply_list;     // PRAND_MT_APPLY_LIST: the position-list application kernel at any size
+    bool mt_apply_list;     // PRAND_MT_APPLY=list: the position-list application kernel at any size
+    bool mt_apply_win;      // PRAND_MT_APPLY=win: the one-stream-per-CTA window kernel instead of four streams per CTA
     int gm_lp;              // PRAND_GM_LP: lanes per GM61 stream (0: default)
     int gm31_nf;            // PRAND_GM31_NF: GM31 points on the FP64 pipe (-1: default 14)
     bool gm_watch_set;      // PRAND_GM_WATCH: limit of the optimistic steps' watch value

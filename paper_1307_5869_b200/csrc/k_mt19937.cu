@@ -18,6 +18,13 @@ constexpr int NW = 624, MW = 397, DEG = 19937;
 
 using prand_dev::mt_recur;
 
+__device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+
 // ---- eq. 10 in correlation form -----------------------------------------------------------------
 // One CTA per destination stream runs the device-callable API's CTA-cooperative skip-ahead
 // (include/prand_device.cuh, mt19937_skipahead_cta: window extension + position-list accumulation).
@@ -109,6 +116,102 @@ mt19937_apply_win_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0
     *reinterpret_cast<uint4 *>(d) = make_uint4(tid == 0 ? (r[0] & 0x80000000u) : r[0], r[1], r[2], r[3]);
 }
 
+// Many destination streams, second form: FOUR streams per CTA share the control flow.  The coefficient word
+// is the same for every thread and every stream, so its bits are consumed two at a time through warp-uniform
+// branches -- nothing is issued for a zero pair, one XOR per output word for a single bit and one three-input
+// XOR for a set pair: 0.75 LOP3 per pair and output word on average instead of the 2 predicated ones above, and
+// the branch instructions are shared by the 16 output words (4 streams x 4 words) of a thread.  Four extended
+// sequences of 82 KB do not fit a CTA, so x is not tabulated: each stream keeps a ring of 1024 words that
+// holds x_{32 wi} .. x_{32 wi + 655}, the part the 156 threads' windows touch at coefficient word wi, and the
+// next 32 words of every stream are generated (by 128 of the threads, recurrence of PAPER.md:374) while word wi
+// is accumulated; one CTA barrier per coefficient word.
+constexpr int AM_S = 4, AM_THREADS = 160, AM_RING = 1024, AM_WB = 8;
+
+// PARAM: the polynomial travels as a kernel argument (2496 bytes of the constant bank): its words, the pair
+// codes and the branch conditions then live on the uniform datapath and cost the ALU pipe nothing.
+template <bool PARAM>
+__global__ void __launch_bounds__(AM_THREADS, 4)
+mt19937_apply_multi_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0, uint64_t count,
+                           uint64_t src_back, const MtOp *__restrict__ op, const __grid_constant__ MtOp opv)
+{
+    __shared__ __align__(16) uint32_t ring[AM_S][AM_RING];
+    const int tid = threadIdx.x;
+    const uint64_t d0 = dst0 + (uint64_t)blockIdx.x * AM_S;
+    const int n_live = (int)(dst0 + count - d0 < (uint64_t)AM_S ? dst0 + count - d0 : AM_S);
+    for (int i = tid; i < AM_S * NW; i += AM_THREADS) {
+        const int q = i / NW, j = i % NW;
+        ring[q][j] = st_src[(d0 + (q < n_live ? q : 0) - src_back) * NW + j];
+    }
+    __syncthreads();
+    // thread g = (stream gq, lane gj) of the generator group extends every ring by 32 words per step
+    const int gq = tid >> 5, gj = tid & 31;
+    auto generate = [&](int k0) {                          // x_{k0 + 624 + gj} from x_{k0 + gj}, +1, +397
+        if (tid < 32 * AM_S) {
+            const int k = k0 + gj;
+            ring[gq][(k + NW) & (AM_RING - 1)] =
+                mt_recur(ring[gq][k & (AM_RING - 1)], ring[gq][(k + 1) & (AM_RING - 1)], ring[gq][(k + MW) & (AM_RING - 1)]);
+        }
+    };
+    generate(0);                                           // x_624 .. x_655
+    __syncthreads();
+    const bool accum = tid < NW / 4;
+    uint32_t acc[AM_S][4] = {};
+    uint32_t pw = PARAM ? 0u : __ldg(&op->w[0]);
+#pragma unroll 1
+    for (int wi = 0; wi < NW; wi++) {
+        const uint32_t p = PARAM ? opv.w[wi] : pw;
+        if (!PARAM && wi + 1 < NW) pw = __ldg(&op->w[wi + 1]);
+        generate(32 * wi + 32);                            // x_{32 wi + 656} .. : the words step wi + 1 adds to the windows
+        if (accum) {
+            // the word's 32 coefficients in AM_WB-bit pieces: a window of AM_WB + 3 (rounded to 4) words per stream
+            // (short windows keep 4 x 4 accumulators + 4 windows at 80 registers: four CTAs per SM, and the piece's
+            // code is executed four times per word instead of being unrolled: 15 KB of instructions)
+#pragma unroll 1
+            for (int h = 0; h < 32; h += AM_WB) {
+                uint32_t v[AM_S][AM_WB + 4];
+#pragma unroll
+                for (int q = 0; q < AM_S; q++)
+#pragma unroll
+                    for (int m = 0; m < (AM_WB + 4) / 4; m++) {
+                        const uint4 t = *reinterpret_cast<const uint4 *>(&ring[q][(32 * wi + h + 4 * tid + 4 * m) & (AM_RING - 1)]);
+                        v[q][4 * m] = t.x; v[q][4 * m + 1] = t.y; v[q][4 * m + 2] = t.z; v[q][4 * m + 3] = t.w;
+                    }
+                const uint32_t ph = p >> h;
+#pragma unroll
+                for (int b = 0; b < AM_WB; b += 2) {
+                    const bool lo = ph & (1u << b), hi = ph & (2u << b);     // warp-uniform
+                    if (lo) {
+                        if (hi) {
+#pragma unroll
+                            for (int q = 0; q < AM_S; q++)
+#pragma unroll
+                                for (int o = 0; o < 4; o++) acc[q][o] = xor3(acc[q][o], v[q][b + o], v[q][b + 1 + o]);
+                        } else {
+#pragma unroll
+                            for (int q = 0; q < AM_S; q++)
+#pragma unroll
+                                for (int o = 0; o < 4; o++) acc[q][o] ^= v[q][b + o];
+                        }
+                    } else if (hi) {
+#pragma unroll
+                        for (int q = 0; q < AM_S; q++)
+#pragma unroll
+                            for (int o = 0; o < 4; o++) acc[q][o] ^= v[q][b + 1 + o];
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+    if (accum) {
+#pragma unroll
+        for (int q = 0; q < AM_S; q++)
+            if (q < n_live)
+                *reinterpret_cast<uint4 *>(st_dst + (d0 + q) * NW + 4 * tid) =
+                    make_uint4(tid == 0 ? (acc[q][0] & 0x80000000u) : acc[q][0], acc[q][1], acc[q][2], acc[q][3]);
+    }
+}
+
 // ---- generation ----------------------------------------------------------------------------------
 // CTA = S adjacent streams x T word slices (thread = (slice t, stream ls), ls fastest).  Thread
 // (t, ls) owns the K = 624/T words w = T j + t, j = 0..K-1, of stream ls and keeps them in registers.
@@ -140,12 +243,6 @@ __device__ __forceinline__ uint32_t lop3_e4(uint32_t a, uint32_t b, uint32_t c) 
 {
     uint32_t d;
     asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
-    return d;
-}
-__device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c)
-{
-    uint32_t d;
-    asm("lop3.b32 %0, %1, %2, %3, 0x96;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
     return d;
 }
 
@@ -986,7 +1083,7 @@ template <int DT> cudaError_t launch_cgen(cudaStream_t stream, const GenArgs &a)
 }  // namespace
 
 cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
-                          uint64_t count, uint64_t src_back, const MtOp *d_op, LaunchInfo *li)
+                          uint64_t count, uint64_t src_back, const MtOp *d_op, const MtOp *h_op, LaunchInfo *li)
 {
     // the opt-in belongs to the current device's context: set it per call (a microsecond), not once per process
     cudaError_t e = cudaFuncSetAttribute(mt19937_apply_kernel<256, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -1009,8 +1106,16 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
         mt19937_apply_kernel<640, 1><<<(unsigned)count, 640, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     else if (debug_hooks().mt_apply_list)                    // test hook: the position-list kernel at any size
         mt19937_apply_kernel<256, 1><<<(unsigned)count, 256, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    else
+    else if (debug_hooks().mt_apply_win || count < 16 * (uint64_t)sm_count())   // (or the test hook) one stream per CTA
         mt19937_apply_win_kernel<<<(unsigned)count, APPLYW_THREADS, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+    else if (h_op)
+        mt19937_apply_multi_kernel<true><<<(unsigned)ceil_div_u64(count, AM_S), AM_THREADS, 0, stream>>>(
+            st_src, st_dst, dst0, count, src_back, d_op, *h_op);
+    else {
+        static const MtOp none = {};
+        mt19937_apply_multi_kernel<false><<<(unsigned)ceil_div_u64(count, AM_S), AM_THREADS, 0, stream>>>(
+            st_src, st_dst, dst0, count, src_back, d_op, none);
+    }
     li->launches = 1;
     return cudaGetLastError();
 }

@@ -64,7 +64,7 @@ void hook_assign(DebugHooks &h, const std::string &name, const char *v)
 {
     const bool on = v && *v;
     if (name == "PRAND_MT_CFG") h.mt_cfg = on ? std::atoi(v) : -1;
-    else if (name == "PRAND_MT_APPLY_LIST") h.mt_apply_list = on;
+    else if (name == "PRAND_MT_APPLY") { h.mt_apply_list = on && std::string(v) == "list"; h.mt_apply_win = on && std::string(v) == "win"; }
     else if (name == "PRAND_GM_LP") h.gm_lp = on ? std::atoi(v) : 0;
     else if (name == "PRAND_GM31_NF") h.gm31_nf = on ? std::atoi(v) : -1;
     else if (name == "PRAND_GM_WATCH") { h.gm_watch_set = on; h.gm_watch = on ? (uint32_t)std::strtoul(v, nullptr, 0) : 0; }
@@ -74,7 +74,7 @@ void hook_assign(DebugHooks &h, const std::string &name, const char *v)
     else if (name == "PRAND_LFSR_INIT") h.lfsr_table = on && std::string(v) == "table";
     else if (name == "PRAND_MT_POLY") h.mt_host_poly = on && std::string(v) == "host";
 }
-const char *const HOOK_NAMES[] = {"PRAND_MT_CFG", "PRAND_MT_APPLY_LIST", "PRAND_GM_LP", "PRAND_GM31_NF", "PRAND_GM_WATCH",
+const char *const HOOK_NAMES[] = {"PRAND_MT_CFG", "PRAND_MT_APPLY", "PRAND_GM_LP", "PRAND_GM31_NF", "PRAND_GM_WATCH",
                                   "PRAND_MRG_INT", "PRAND_GM_INIT", "PRAND_CHUNK_LEN", "PRAND_LFSR_INIT", "PRAND_MT_POLY"};
 void hooks_from_env()
 {
@@ -355,13 +355,13 @@ int init_mt19937(prand_state *st, uint64_t seed, Dist L, cudaStream_t stream, co
     const MtOp *d_ops = (const MtOp *)st->d_ops;
     LaunchInfo li;
     if (have_first) {
-        CU(mt19937_apply(stream, d, d, 0, 1, 0, d_ops + lev_tree, &li));
+        CU(mt19937_apply(stream, d, d, 0, 1, 0, d_ops + lev_tree, &ops[lev_tree], &li));
         note(st, li);
     }
     for (unsigned j = 0; j < lev_tree; j++) {
         uint64_t lo = 1ull << j;
         uint64_t count = st->ns - lo < lo ? st->ns - lo : lo;
-        CU(mt19937_apply(stream, d, d, lo, count, lo, d_ops + j, &li));
+        CU(mt19937_apply(stream, d, d, lo, count, lo, d_ops + j, &ops[j], &li));
         note(st, li);
     }
     return PRAND_OK;
@@ -517,7 +517,7 @@ int jump_launch(prand_state *st, cudaStream_t stream, const Dist *dist = nullptr
     LaunchInfo li;
     if (st->gen == PRAND_MT19937) {
         uint32_t *d = (uint32_t *)st->d_state[st->cur];
-        CU(mt19937_apply(stream, d, d, 0, st->ns, 0, (const MtOp *)st->d_ops, &li));
+        CU(mt19937_apply(stream, d, d, 0, st->ns, 0, (const MtOp *)st->d_ops, nullptr, &li));
     } else {
         JumpArgs a;
         a.base = nullptr;
@@ -557,7 +557,7 @@ extern "C" int prand_jump(prand_state *st, uint64_t steps_mant, unsigned steps_l
                 uint32_t *d = (uint32_t *)st->d_state[st->cur];
                 for (int t : terms) {
                     LaunchInfo li;
-                    CU(mt19937_apply(stream, d, d, 0, st->ns, 0, table + t, &li));
+                    CU(mt19937_apply(stream, d, d, 0, st->ns, 0, table + t, (const MtOp *)host::mt19937_table() + t, &li));
                     li.kernel = "mt19937_apply<table>";
                     note(st, li);
                 }
