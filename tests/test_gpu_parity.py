@@ -318,6 +318,62 @@ def test_set_state_refuses_words_the_kernels_cannot_take():
     assert P.lib().prand_trim() == 0
 
 
+@pytest.mark.parametrize("hook", [None, "win", "list"])
+def test_mt19937_every_polynomial_application_kernel(hook):
+    """Eq. 10 in all its kernels: the four-streams-per-CTA form with the polynomial as a
+    kernel argument (tree levels of >= 2368 streams) and from device memory (prand_jump by a distance that is
+    not tabulated), the one-stream window form and the position-list form (hooks), the 640-thread and the
+    4-CTA split forms of the small levels.  Sampled streams against the oracle."""
+    need_gpu()
+    ns, L, steps = 6000, 2**64, (2**40 + 12345) << 480
+    P.prand_debug_set("PRAND_MT_APPLY", hook)
+    try:
+        g = P.Generator("mt19937", 5489, ns, L)
+        g.jump(steps)
+        got = g.generate(40, "u32").cpu().numpy().view(np.uint32)
+        st = g.state()
+        g.close()
+    finally:
+        P.prand_debug_set("PRAND_MT_APPLY", None)
+    sb = oracle.state_bytes("mt19937")
+    for s in (0, 2047, 2048, 4096, ns - 1):
+        want, wst = oracle.streams("mt19937", 5489, s, 1, L, 40, "u32", pre_jump=steps)
+        assert np.array_equal(got[:, s], want[:, 0]), (hook, s)
+        assert st[s * sb:(s + 1) * sb] == wst.tobytes(), (hook, s)
+
+
+@pytest.mark.parametrize("cfg", range(4))
+def test_shared_memory_kernels_repeat_bit_for_bit(cfg):
+    """compute-sanitizer is not available on this GPU pool, so races in the shared-memory MT19937 kernels (in-place
+    circular windows, deferred tempering, split cluster barriers, cp.async state loads, DSMEM bulk copies) are hunted
+    by repetition instead: every kernel variant runs eight times from the same state at a size that fills the GPU,
+    and all runs must agree bit for bit with the first, which is checked against the oracle on sampled streams."""
+    need_gpu()
+    ns = {0: 4736, 1: 1184, 2: 592, 3: 592}[cfg]           # 148 CTAs of 32 / 8 / 4 / 4 streams
+    n = 624 * 9 + 77
+    P.prand_debug_set("PRAND_MT_CFG", str(cfg))
+    try:
+        g = P.Generator("mt19937", 5489, ns, 2**64)
+        start = g.state()
+        first = None
+        for rep in range(8):
+            g.set_state(start)
+            out = g.generate(n, "u32")
+            assert g.last_kernel == MT_CFG_KERNEL[cfg]
+            if first is None:
+                first, first_state = out.clone(), g.state()
+            else:
+                assert torch.equal(out, first), f"run {rep} differs from run 0"
+                assert g.state() == first_state
+        g.close()
+    finally:
+        P.prand_debug_set("PRAND_MT_CFG", None)
+    got = first.cpu().numpy().view(np.uint32)
+    for s in (0, ns // 2 + 1, ns - 1):
+        want, _ = oracle.streams("mt19937", 5489, s, 1, 2**64, n, "u32")
+        assert np.array_equal(got[:, s], want[:, 0]), s
+
+
 def test_mt19937_jumps_use_the_precomputed_polynomial_table():
     """tabulated distances (2^n, n < 512; m 2^i, m = 15..24, i < 128) are one application of a
     device-resident polynomial; other distances are applied term by term of their binary notation; distances
