@@ -335,10 +335,11 @@ mrg32k3a_seq_f64_kernel(const uint32_t *st_in, uint32_t *st_last, double *__rest
             }
         }
         __syncwarp();
-        const int sub = lane >> 3, piece = lane & 7;
+        constexpr int LPS = SEQ_ROWS / 2;                  // lanes per section: each stores two doubles
+        const int sub = lane / LPS, piece = lane % LPS;
 #pragma unroll 4
-        for (int k = 0; k < 8 * V; k++) {
-            const int sl = 4 * k + sub;                    // section within the warp
+        for (int k = 0; k < 32 * V / (32 / LPS); k++) {
+            const int sl = (32 / LPS) * k + sub;           // section within the warp
             const uint64_t sec = warp_sec0 + sl;
             const uint64_t row = i0 + 2 * piece;
             if (sec < n_sections) {

@@ -792,6 +792,7 @@ void plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec
     // enough sections to fill the GPU, sections long enough to amortise the jump to their start
     const uint64_t min_len = gen == PRAND_MT19937 ? 8 * 624 : 1024;
     // MT19937: every section costs a polynomial application (~1 us of a whole SM): one CTA of four sections per SM
+    // others: one section per thread; 2^17 sections are one wave of 28 warps per SM on 148 SMs
     const uint64_t max_sec = gen == PRAND_MT19937 ? 4 * (uint64_t)sms : 131072;
     uint64_t S = length / min_len;
     if (S > max_sec) S = max_sec;
