@@ -8,6 +8,7 @@
 // output number P = temper(x_{P+624}); the state at position P is the window x_P..x_{P+623}.
 // State layout: [stream][624] u32 (one stream's window is contiguous: a warp loads it coalesced).
 #include <cstdlib>
+#include <cuda.h>                                         // CUtensorMap (types only: the encoder comes through the runtime)
 #include "k_common.cuh"
 #include "../../include/prand_device.cuh"
 
@@ -433,6 +434,200 @@ template <int S, int T, int M, int HI, bool PAIR> cudaError_t dispatch_dt(cudaSt
     case DT_U32: return launch_gen<S, T, M, DT_U32, HI, PAIR>(stream, a);
     case DT_F32: return launch_gen<S, T, M, DT_F32, HI, PAIR>(stream, a);
     default: return launch_gen<S, T, M, DT_F64, HI, PAIR>(stream, a);
+    }
+}
+
+// ---- generation, few streams: rows leave through TMA tensor stores ------------------------------------
+// Same CTA = S streams x T word slices and the same rounds as above, but a number is not stored to global
+// memory by its thread: a CTA that writes 16-byte pieces of a row (S = 4, four-byte outputs) is bound by the
+// SM's store path -- measured on C3's geometry (128 CTAs, 2048-byte rows, profiles/r02_store_pieces.md):
+// STG 2.0 TB/s, TMA tensor stores of [rows x 16 bytes] boxes 3.3 TB/s.  The tempered number goes to a
+// shared-memory tile [M T rows][S streams] instead (tile index = thread index: conflict-free), and once the
+// CTA barrier that the recurrence needs anyway has passed, one thread sends the tile with a single
+// cp.async.bulk.tensor.2d store (box = S elements x M T rows).  Tiles: two rounds' worth (2 K/M buffers);
+// the issuing thread waits (wait_group.read) until the store that last used the next buffer has read it.
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap *tm, uint32_t src, int x, int y)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 :: "l"(tm), "r"(x), "r"(y), "r"(src) : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+
+template <int S, int T, int M, int DT, int HI, bool PAIR>
+__global__ void __launch_bounds__(S * T)
+mt19937_tgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT>::type *__restrict__ out,
+                    uint64_t ns, uint64_t n, const MtMul c, const __grid_constant__ CUtensorMap tmap)
+{
+    typedef typename OutElem<DT>::type E;
+    constexpr int K = NW / T, P = MtPitch<S>::value, NT = S * T, NG = K / M, TILE = M * NT;
+    constexpr int W32 = (int)(sizeof(E) / 4);             // 32-bit words per element (the tensor map counts words)
+    static_assert(NW % T == 0 && K % M == 0 && T * M <= NW - MW && M * T <= 256, "bad MT19937 tiling");
+    static_assert((2 * S * P * 4) % 128 == 0 && (TILE * sizeof(E)) % 128 == 0, "tiles must be 128-byte aligned");
+    extern __shared__ __align__(128) uint32_t smem[];     // windows [2][S][P], tiles [2 NG][TILE] of E
+    E *tiles = reinterpret_cast<E *>(smem + 2 * S * P);
+    const int tid = threadIdx.x, ls = tid % S, t = tid / S;
+    const uint64_t s0 = (uint64_t)blockIdx.x * S;
+    const uint64_t s = s0 + ls;
+    const bool live = s < ns;
+    const int n_live = s0 >= ns ? 0 : (ns - s0 < (uint64_t)S ? (int)(ns - s0) : S);
+    const bool issuer = tid == 0 && n_live > 0;
+
+    for (int i = tid; i < S * (NW / 4); i += NT) {
+        const int q = i / (NW / 4), w4 = i % (NW / 4);
+        if (q < n_live) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4 *>(st_in + (s0 + q) * NW) + w4);
+            *reinterpret_cast<uint4 *>(smem + q * P + 4 * w4) = v;
+        }
+    }
+    __syncthreads();
+    uint32_t ia = ls * P + t, ib = ia + S * P;
+    uint32_t r[K];
+#pragma unroll
+    for (int j = 0; j < K; j++) r[j] = smem[ia + T * j];
+    const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tiles);
+    uint32_t ta = 0, tb = NG * TILE;                      // element offsets of this round's / the other round's tiles
+    const int x = (int)(s0 * W32);
+    const uint32_t rounds = (uint32_t)(n / NW);           // the launcher keeps n below 2^31
+    const int rem = (int)(n % NW);
+    uint32_t pend = 0;
+    bool pending = false;
+    int y = 0;                                            // first row of the round
+    for (uint32_t rd = 0; rd < rounds; rd++) {
+#pragma unroll
+        for (int j = 0; j < K; j++) {
+            const uint32_t x1 = smem[ia + T * j + 1];
+            uint32_t xm;
+            if (T * (j + 1) <= NW - MW) xm = smem[ia + T * j + MW];
+            else if (T * j >= NW - MW) xm = smem[ib + T * j - (NW - MW)];
+            else xm = smem[(T * j + t < NW - MW ? ia + MW : ib - (NW - MW)) + T * j];
+            // the previous wave's number: tempering and tile store fill the wait for this wave's operands
+            if (j != 0 || rd != 0) {
+                const int q = (j + K - 1) % K;
+                tiles[(j == 0 ? tb : ta) + (q / M) * TILE + (q % M) * NT + tid] = convert<DT>(mt_temper2<HI>(pend, c));
+            }
+            const uint32_t nw = mt_recur2<HI>(r[j], x1, xm, c);
+            r[j] = nw;
+            smem[ib + T * j] = nw;
+            if (j == 0 && t == 0) smem[ia + NW] = nw;       // x_{w+1} of word 623 is the new word 0
+            pend = nw;
+            if ((j + 1) % M == 0) {
+                const int gg = j / M;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // tile writes -> visible to the TMA engine
+                if (issuer && !(dbg & 2)) asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(2 * NG - 3) : "memory");
+                __syncthreads();
+                // the tile of the previous group is complete
+                if (issuer && (gg != 0 || rd != 0) && !(dbg & 4)) {
+                    if (dbg & 1) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                    const int pg = (gg + NG - 1) % NG;
+                    tma_store_2d(&tmap, tile_s + (uint32_t)(((gg == 0 ? tb : ta) + pg * TILE) * sizeof(E)), x,
+                                 y + (gg == 0 ? -NW : 0) + pg * M * T);
+                }
+            }
+        }
+        if (PAIR) {                                       // stay within one round of the sector partner
+            if (pending) cluster_wait();
+            cluster_arrive();
+            pending = true;
+        }
+        { const uint32_t tmp = ia; ia = ib; ib = tmp; }
+        { const uint32_t tmp = ta; ta = tb; tb = tmp; }
+        y += NW;
+    }
+    if (rounds) {                                         // the last wave's number and the last tile
+        tiles[tb + (NG - 1) * TILE + ((K - 1) % M) * NT + tid] = convert<DT>(mt_temper2<HI>(pend, c));
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (issuer) tma_store_2d(&tmap, tile_s + (uint32_t)((tb + (NG - 1) * TILE) * sizeof(E)), x, y - NW + (NG - 1) * M * T);
+    }
+    if (PAIR && pending) cluster_wait();
+    // ragged tail (< 624 rows): straight to global memory
+    if (rem) {
+        const uint32_t ob = (uint32_t)(((uint64_t)t * ns + ls) * sizeof(E));
+        char *rows = reinterpret_cast<char *>(out + s0) + (uint64_t)rounds * NW * ns * sizeof(E);
+        E *pend_p = nullptr;
+        mt_round<S, T, M, DT, HI, false, false, false>(smem, ia, ib, t, r, rows, ob, (uint64_t)T * ns * sizeof(E), live,
+                                                       rem, c, pend, pend_p);
+    }
+    // final window x_{P+n}..x_{P+n+623}: words [rem, 624) of the old buffer, then [0, rem) of the new
+    const uint32_t cur = rounds & 1;
+    const uint32_t *a0 = smem + cur * (S * P), *b0 = smem + (cur ^ 1) * (S * P);
+    for (int i = tid; i < S * NW; i += NT) {
+        const int q = i / NW, j = i % NW;
+        if (q < n_live) {
+            const int p = j + rem;
+            st_out[(s0 + q) * NW + j] = p < NW ? a0[q * P + p] : b0[q * P + p - NW];
+        }
+    }
+    if (issuer) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");     // the tiles outlive the stores' reads
+}
+
+typedef CUresult (*TensorMapEncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                      const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// cuTensorMapEncodeTiled through the runtime (libprand does not link libcuda); nullptr if the driver has none
+TensorMapEncodeFn tensor_map_encoder()
+{
+    static TensorMapEncodeFn fn = [] {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        return (TensorMapEncodeFn)p;
+    }();
+    return fn;
+}
+
+// the TMA path needs 16-byte aligned rows of at most 2^31 - 1 and at least one full round
+bool tgen_ok(const GenArgs &a)
+{
+    return a.n_streams % 4 == 0 && (uintptr_t)a.out % 16 == 0 && a.n >= NW && a.n < (1ull << 31) && tensor_map_encoder();
+}
+
+template <int S, int T, int M, int DT, int HI, bool PAIR> cudaError_t launch_tgen(cudaStream_t stream, const GenArgs &a)
+{
+    typedef typename OutElem<DT>::type E;
+    auto kern = mt19937_tgen_kernel<S, T, M, DT, HI, PAIR>;
+    constexpr int K = NW / T, NG = K / M;
+    const size_t smem = (size_t)2 * S * MtPitch<S>::value * sizeof(uint32_t) + (size_t)2 * NG * M * S * T * sizeof(E);
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    // the output as a 2-D tensor of 32-bit words: [rows of full rounds][n_streams * words per element]
+    const uint32_t w32 = (uint32_t)(sizeof(E) / 4);
+    CUtensorMap tm;
+    const cuuint64_t dims[2] = {a.n_streams * w32, (a.n / NW) * NW};
+    const cuuint64_t strides[1] = {a.n_streams * sizeof(E)};
+    const cuuint32_t box[2] = {S * w32, (cuuint32_t)(M * T)};
+    const cuuint32_t es[2] = {1, 1};
+    if (tensor_map_encoder()(&tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, a.out, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorInvalidValue;
+    uint64_t blocks = ceil_div_u64(a.n_streams, S);
+    if (PAIR) blocks += blocks & 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)blocks);
+    cfg.blockDim = dim3(S * T);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = PAIR ? 2 : 1;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    const MtMul c = {2u * 0x1908B0DFu, 1u << 31, 1u << 21, 1u << 14};
+    return cudaLaunchKernelEx(&cfg, kern, (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (E *)a.out, a.n_streams, a.n, c, tm);
+}
+
+template <int S, int T, int M, int HI, bool PAIR> cudaError_t dispatch_tdt(cudaStream_t stream, const GenArgs &a)
+{
+    switch (a.dtype) {
+    case DT_U32: return launch_tgen<S, T, M, DT_U32, HI, PAIR>(stream, a);
+    case DT_F32: return launch_tgen<S, T, M, DT_F32, HI, PAIR>(stream, a);
+    default: return launch_tgen<S, T, M, DT_F64, HI, PAIR>(stream, a);
     }
 }
 
@@ -944,6 +1139,227 @@ mt19937_cgen_kernel(const uint32_t *st_in, uint32_t *st_out, uint32_t *__restric
     }
 }
 
+// ---- generation, few streams: warp = stream, window in registers, rows leave through TMA ----------------
+// With a few hundred streams (C3: 512 = 4 per SM on 128 SMs) the slice kernels above are bound by their own
+// instruction stream and by latency, not by any pipe: a wave of 208 words per stream is one shared-memory
+// round trip, a dozen dependent instructions and a CTA barrier, every warp of the CTA waits for the same thing
+// at the same time, and the per-wave bookkeeping costs more issue slots than the arithmetic (ncu: 1.09 ms on
+// C3 even with the stores removed).  Here a WARP owns a stream and the recurrence shares nothing: the window
+// lives in registers, word i of the sequence in lane i mod 32 of ring slot (i / 32) mod 20 (640 words: the
+// window and the 16 words that complete its last slot).  A step produces the 32 words of one slot, lane l from
+// x_{i-624}, x_{i-623}, x_{i-227} -- lanes l+16, l+17, l+29 (mod 32) of slots k / k+1 resp. k+12 / k+13: three
+// selects and three shuffles, no shared memory, no barrier; the seven steps before a step are independent of it
+// (227 > 7 * 32), which is the instruction-level parallelism a lone warp needs.  One turn of the ring (20 steps,
+// 640 rows) is unrolled.
+// One warp per scheduler can issue only every other clock (measured: 2.2 clocks per instruction at best), so the
+// work of a number is split over two warps on the same scheduler: the COMPUTE warp of a stream runs the
+// recurrence alone (12 instructions per 32 numbers) and drops the raw words into a staging column
+// [stream][640 rows]; four HELPER warps take a quarter of the rows each, read the four streams' words of a row,
+// temper and convert them and write the row as one 16-byte piece into a tile of their own -- [160 rows][4
+// streams], conflict-free both ways -- which the same warp sends with one TMA tensor store (box 160 rows x 16
+// bytes: 3.3 TB/s on C3's geometry against 2.0 TB/s for 16-byte STG pieces, profiles/r02_store_pieces.md).
+// Only the staging buffers are handed over (two mbarriers each, generic proxy, no fence); a helper waits for its
+// own TMA stores (bulk groups are per thread), so nobody fences or waits on the compute warps' path.  Rows
+// outside whole turns of the ring (the first 16, the last < 640) take a plain warp-level path on a
+// shared-memory copy of the ring.
+constexpr int WG_S = 4;                                   // streams = compute warps = helper warps per CTA
+constexpr int WG_RING = 20;                               // ring slots (registers per lane)
+constexpr int WG_XS = 32 * WG_RING;                       // 640 words = rows per turn
+constexpr int WG_BOX = WG_XS / WG_S;                      // rows per helper and turn: one TMA box
+constexpr int WG_NSB = 3;                                 // staging buffers
+constexpr int WG_NTB = 4;                                 // tile buffers per helper
+constexpr int WG_THREADS = 64 * WG_S;
+static_assert(WG_BOX % 32 == 0 && WG_BOX <= 256 && (WG_BOX * WG_S * 4) % 128 == 0, "bad tile");
+
+// rows [ra, rb) of one stream by its warp, ring in shared memory (word i of the call at xs[i mod 640])
+template <int DT>
+__device__ __forceinline__ void wg_slow_rows(uint32_t *xs, uint64_t ra, uint64_t rb, typename OutElem<DT>::type *col,
+                                             uint64_t ns, int lane, const MtMul &c)
+{
+    uint32_t pos = (uint32_t)(ra % WG_XS);
+    for (uint64_t r0 = ra; r0 < rb; r0 += 32) {
+        const bool on = r0 + lane < rb;
+        uint32_t a0 = pos + lane;
+        a0 -= a0 >= WG_XS ? WG_XS : 0;
+        uint32_t a1 = a0 + 1, am = a0 + MW, aw = a0 + NW;
+        a1 -= a1 >= WG_XS ? WG_XS : 0;
+        am -= am >= WG_XS ? WG_XS : 0;
+        aw -= aw >= WG_XS ? WG_XS : 0;
+        uint32_t nw = 0;
+        if (on) nw = mt_recur2<0>(xs[a0], xs[a1], xs[am], c);
+        __syncwarp();                                      // every operand read before any cell is rewritten
+        if (on) {
+            xs[aw] = nw;
+            store1(col + (r0 + lane) * ns, convert<DT>(mt_temper2<0>(nw, c)));
+        }
+        __syncwarp();
+        pos += 32;
+        pos -= pos >= WG_XS ? WG_XS : 0;
+    }
+}
+
+__device__ __forceinline__ void wg_store_row(uint32_t *p, const uint32_t (&v)[4])
+{
+    *reinterpret_cast<uint4 *>(p) = make_uint4(v[0], v[1], v[2], v[3]);
+}
+__device__ __forceinline__ void wg_store_row(float *p, const float (&v)[4])
+{
+    *reinterpret_cast<float4 *>(p) = make_float4(v[0], v[1], v[2], v[3]);
+}
+__device__ __forceinline__ void wg_store_row(double *p, const double (&v)[4])
+{
+    *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[1]);
+    *reinterpret_cast<double2 *>(p + 2) = make_double2(v[2], v[3]);
+}
+
+template <int DT, int HI>
+__global__ void __launch_bounds__(WG_THREADS, 1)
+mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT>::type *__restrict__ out,
+                    uint64_t ns, uint64_t n, const MtMul c, const __grid_constant__ CUtensorMap tmap)
+{
+    typedef typename OutElem<DT>::type E;
+    constexpr int W32 = (int)(sizeof(E) / 4);
+    constexpr int TILE = WG_BOX * WG_S;                   // elements per helper tile
+    // tiles [helper][NTB][TILE] of E, staging [NSB][stream][640], rings [stream][640], mbarriers sfull[NSB], sempty[NSB]
+    extern __shared__ __align__(128) uint32_t smem[];
+    E *tiles = reinterpret_cast<E *>(smem);
+    uint32_t *staging = smem + WG_S * WG_NTB * TILE * W32;
+    uint32_t *rings = staging + WG_NSB * WG_S * WG_XS;
+    const uint32_t bars = smem_addr(rings + WG_S * WG_XS);
+    const uint32_t sfull = bars, sempty = bars + 8 * WG_NSB;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint64_t s0 = (uint64_t)blockIdx.x * WG_S;
+    if (s0 >= ns) return;                                 // (the launcher guarantees ns % 4 == 0: a CTA is whole or dead)
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < WG_NSB; b++) {
+            mbar_init(sfull + 8 * b, WG_S);
+            mbar_init(sempty + 8 * b, WG_S);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const uint32_t turns = n >= 16 ? (uint32_t)((n - 16) / WG_XS) : 0;   // whole turns of the ring after the first 16 rows
+
+    if (warp >= WG_S) {
+        // ---- helper warp h: rows [160 h, 160 h + 160) of every turn, all four streams ----------------------
+        const int h = warp - WG_S;
+        E *my = tiles + h * WG_NTB * TILE;
+        const uint32_t my_s = smem_addr(my);
+        const int x = (int)(s0 * W32);
+        for (uint32_t u = 0; u < turns; u++) {
+            const uint32_t b = u % WG_NSB, tb = u % WG_NTB;
+            if (lane == 0) {
+                mbar_wait(sfull + 8 * b, (u / WG_NSB) & 1u);
+                if (u >= WG_NTB) asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(WG_NTB - 1) : "memory");
+            }
+            __syncwarp();
+            const uint32_t *sp = staging + b * (WG_S * WG_XS) + h * WG_BOX + lane;
+            E *tp = my + tb * TILE + lane * WG_S;
+#pragma unroll
+            for (int i = 0; i < WG_BOX / 32; i++) {
+                E v[WG_S];
+#pragma unroll
+                for (int q = 0; q < WG_S; q++) v[q] = convert<DT>(mt_temper2<HI>(sp[q * WG_XS + 32 * i], c));
+                wg_store_row(tp + 32 * i * WG_S, v);
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // tile writes -> visible to the TMA engine
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(sempty + 8 * b);
+                tma_store_2d(&tmap, my_s + tb * (uint32_t)(TILE * sizeof(E)), x, 16 + WG_XS * (int)u + WG_BOX * h);
+            }
+        }
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        return;
+    }
+
+    // ---- compute warp g: stream s0 + g ----------------------------------------------------------------------
+    const int g = warp;
+    uint32_t *xs = rings + g * WG_XS;
+    {
+        const uint32_t *src = st_in + (s0 + g) * NW;
+        for (int i = lane; i < NW; i += 32) xs[i] = __ldg(src + i);
+    }
+    __syncwarp();
+    E *col = out + s0 + g;
+    wg_slow_rows<DT>(xs, 0, n < 16 ? n : 16, col, ns, lane, c);
+    if (turns) {
+        uint32_t r[WG_RING];
+#pragma unroll
+        for (int q = 0; q < WG_RING; q++) r[q] = xs[32 * q + lane];
+        const bool ge16 = lane >= 16, ge17 = lane >= 17, ge29 = lane >= 29;
+        const int l17 = (lane + 17) & 31, l29 = (lane + 29) & 31;
+        for (uint32_t u = 0; u < turns; u++) {
+            const uint32_t b = u % WG_NSB;
+            if (u >= WG_NSB) {
+                if (lane == 0) mbar_wait(sempty + 8 * b, ((u / WG_NSB) - 1u) & 1u);
+                __syncwarp();
+            }
+            uint32_t *sp = staging + (b * WG_S + g) * WG_XS + lane;
+#pragma unroll
+            for (int k = 0; k < WG_RING; k++) {
+                const uint32_t v0 = ge16 ? r[k] : r[(k + 1) % WG_RING];
+                const uint32_t v1 = ge17 ? r[k] : r[(k + 1) % WG_RING];
+                const uint32_t vm = ge29 ? r[(k + 12) % WG_RING] : r[(k + 13) % WG_RING];
+                const uint32_t x0 = __shfl_xor_sync(0xffffffffu, v0, 16);
+                const uint32_t x1 = __shfl_sync(0xffffffffu, v1, l17);
+                const uint32_t xm = __shfl_sync(0xffffffffu, vm, l29);
+                const uint32_t nw = mt_recur2<HI>(x0, x1, xm, c);
+                r[k] = nw;
+                sp[32 * k] = nw;
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(sfull + 8 * b);
+        }
+#pragma unroll
+        for (int q = 0; q < WG_RING; q++) xs[32 * q + lane] = r[q];
+        __syncwarp();
+    }
+    wg_slow_rows<DT>(xs, n < 16 ? n : 16 + (uint64_t)turns * WG_XS, n, col, ns, lane, c);
+    // the window after n numbers: words n .. n + 623 of the call
+    {
+        uint32_t *dst = st_out + (s0 + g) * NW;
+        uint32_t pos = (uint32_t)(n % WG_XS) + lane;
+        for (int i = lane; i < NW; i += 32) {
+            pos -= pos >= WG_XS ? WG_XS : 0;
+            dst[i] = xs[pos];
+            pos += 32;
+        }
+    }
+}
+
+template <int DT, int HI> cudaError_t launch_wgen(cudaStream_t stream, const GenArgs &a)
+{
+    typedef typename OutElem<DT>::type E;
+    auto kern = mt19937_wgen_kernel<DT, HI>;
+    const size_t smem = (size_t)WG_S * WG_NTB * WG_BOX * WG_S * sizeof(E) + (size_t)(WG_NSB + 1) * WG_S * WG_XS * 4 + 2 * WG_NSB * 8;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const uint32_t w32 = (uint32_t)(sizeof(E) / 4);
+    CUtensorMap tm;
+    const cuuint64_t dims[2] = {a.n_streams * w32, a.n};
+    const cuuint64_t strides[1] = {a.n_streams * sizeof(E)};
+    const cuuint32_t box[2] = {WG_S * w32, WG_BOX};
+    const cuuint32_t es[2] = {1, 1};
+    if (tensor_map_encoder()(&tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, a.out, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                             CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorInvalidValue;
+    const MtMul c = {2u * 0x1908B0DFu, 1u << 31, 1u << 21, 1u << 14};
+    kern<<<(unsigned)ceil_div_u64(a.n_streams, WG_S), WG_THREADS, smem, stream>>>(
+        (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (E *)a.out, a.n_streams, a.n, c, tm);
+    return cudaGetLastError();
+}
+
+template <int HI> cudaError_t dispatch_wdt(cudaStream_t stream, const GenArgs &a)
+{
+    switch (a.dtype) {
+    case DT_U32: return launch_wgen<DT_U32, HI>(stream, a);
+    case DT_F32: return launch_wgen<DT_F32, HI>(stream, a);
+    default: return launch_wgen<DT_F64, HI>(stream, a);
+    }
+}
+
 // ---- sections of a single sequence (prand_generate_seq_*; Table 5) ----------------------
 // Section c = stream c of the family, its numbers contiguous in memory: out[c * sec_len + i].  With the
 // per-stream thread groups of the kernel above (thread = two adjacent words of a wave, 104 threads per
@@ -1147,7 +1563,7 @@ cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *
     // bound by the ~10-13 B/clk/SM that distributed shared memory moves between four CTAs)
     if (debug_hooks().mt_cfg >= 0) {                                          // test hook: force a variant
         const int want = debug_hooks().mt_cfg;
-        if (want != 3 || gather_ok) cfg = want;
+        if ((want != 3 || gather_ok) && (want < 4 || tgen_ok(a))) cfg = want;
     }
     switch (cfg) {
     case 0: li->kernel = "mt19937_bgen<S=32>"; return dispatch_bdt<0>(stream, a);
@@ -1155,6 +1571,10 @@ cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *
     case 3:
         li->kernel = "mt19937_cgen<CS=4>";
         return a.dtype == DT_U32 ? launch_cgen<DT_U32>(stream, a) : launch_cgen<DT_F32>(stream, a);
+    case 6: li->kernel = "mt19937_wgen<S=4>"; return dispatch_wdt<6>(stream, a);
+    case 7: li->kernel = "mt19937_wgen<S=4>"; return dispatch_wdt<0>(stream, a);
+    case 4: li->kernel = "mt19937_tgen<S=4,T=208,pair>"; return dispatch_tdt<4, 208, 1, 6, true>(stream, a);
+    case 5: li->kernel = "mt19937_tgen<S=8,T=104>"; return dispatch_tdt<8, 104, 2, 0, false>(stream, a);
     default: li->kernel = "mt19937_gen<S=4,T=208,pair>"; return dispatch_dt<4, 208, 1, 6, true>(stream, a);
     }
 }
