@@ -559,6 +559,30 @@ def run_pipe_rates(args):
     print(json.dumps({"pipe_rates": rows, "sms": sms}), flush=True)
 
 
+# ---- store pieces of few-stream kernels (profiles/r02_store_pieces.md) -------------------------------------
+def run_store_probe(args):
+    """2^20 rows of 2048 bytes (C3's output) written as 16-byte pieces by 128 CTAs resp. 32-byte pieces by 64 CTAs,
+    with STG and with TMA tensor stores, and how the time grows when partner CTAs start `skew` clocks apart."""
+    import torch
+    import paper_1307_5869_b200 as P
+
+    torch.cuda.set_device(0)
+    rows = (1 << 20) // 160 * 160
+    buf = torch.empty(rows * 2048, dtype=torch.uint8, device="cuda")
+    out = []
+    for method, mname in ((0, "stg"), (1, "tma")):
+        for pb, g in ((16, 128), (32, 64), (64, 32)):
+            for mode in (0, 1, 2, 3):
+                for skew in ((0,) if mode == 0 else (500, 2000, 10000, 50000)):
+                    def fn():
+                        P.prand_probe_store_pieces(buf.data_ptr(), buf.numel(), method, pb, g, rows, skew, mode)
+                    ms = statistics.median(event_ms(torch, fn, 5, warm=2))
+                    delay_ms = {0: 0, 1: 1, 2: 7, 3: 3}[mode] * skew / 1.965e6
+                    out.append({"method": mname, "piece_bytes": pb, "ctas": g, "skew_mode": mode, "skew_clocks": skew,
+                                "ms": ms, "ms_net_of_start_delay": ms - delay_ms, "gbs": rows * 2048 / (ms - delay_ms) / 1e6})
+    print(json.dumps({"store_pieces": out, "rows": rows, "row_bytes": 2048}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     ap.add_argument("--gpus", type=int, default=1)
@@ -573,12 +597,15 @@ def main():
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config table (all other configs)")
     ap.add_argument("--config-steps", type=int, default=10, help="timed calls per per_config row")
     ap.add_argument("--pipe-rates", action="store_true", help="print the SM pipe instruction rates (probe kernels)")
+    ap.add_argument("--store-probe", action="store_true", help="print the store-piece probe table (profiles/r02_store_pieces.md)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours" and not args.sweep:
         args.warmup = 3                          # timing rule: at least three warm-up steps
     w = workloads.ALL[args.workload]
     if args.pipe_rates:
         return run_pipe_rates(args)
+    if args.store_probe:
+        return run_store_probe(args)
     if args.sweep:
         return run_sweep(args)
     if args.impl == "reference":

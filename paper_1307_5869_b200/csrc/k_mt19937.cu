@@ -513,11 +513,10 @@ mt19937_tgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
             if ((j + 1) % M == 0) {
                 const int gg = j / M;
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // tile writes -> visible to the TMA engine
-                if (issuer && !(dbg & 2)) asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(2 * NG - 3) : "memory");
+                if (issuer) asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(2 * NG - 3) : "memory");
                 __syncthreads();
                 // the tile of the previous group is complete
-                if (issuer && (gg != 0 || rd != 0) && !(dbg & 4)) {
-                    if (dbg & 1) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                if (issuer && (gg != 0 || rd != 0)) {
                     const int pg = (gg + NG - 1) % NG;
                     tma_store_2d(&tmap, tile_s + (uint32_t)(((gg == 0 ? tb : ta) + pg * TILE) * sizeof(E)), x,
                                  y + (gg == 0 ? -NW : 0) + pg * M * T);
@@ -1144,32 +1143,63 @@ mt19937_cgen_kernel(const uint32_t *st_in, uint32_t *st_out, uint32_t *__restric
 // instruction stream and by latency, not by any pipe: a wave of 208 words per stream is one shared-memory
 // round trip, a dozen dependent instructions and a CTA barrier, every warp of the CTA waits for the same thing
 // at the same time, and the per-wave bookkeeping costs more issue slots than the arithmetic (ncu: 1.09 ms on
-// C3 even with the stores removed).  Here a WARP owns a stream and the recurrence shares nothing: the window
-// lives in registers, word i of the sequence in lane i mod 32 of ring slot (i / 32) mod 20 (640 words: the
-// window and the 16 words that complete its last slot).  A step produces the 32 words of one slot, lane l from
-// x_{i-624}, x_{i-623}, x_{i-227} -- lanes l+16, l+17, l+29 (mod 32) of slots k / k+1 resp. k+12 / k+13: three
-// selects and three shuffles, no shared memory, no barrier; the seven steps before a step are independent of it
-// (227 > 7 * 32), which is the instruction-level parallelism a lone warp needs.  One turn of the ring (20 steps,
-// 640 rows) is unrolled.
-// One warp per scheduler can issue only every other clock (measured: 2.2 clocks per instruction at best), so the
-// work of a number is split over two warps on the same scheduler: the COMPUTE warp of a stream runs the
-// recurrence alone (12 instructions per 32 numbers) and drops the raw words into a staging column
-// [stream][640 rows]; four HELPER warps take a quarter of the rows each, read the four streams' words of a row,
-// temper and convert them and write the row as one 16-byte piece into a tile of their own -- [160 rows][4
-// streams], conflict-free both ways -- which the same warp sends with one TMA tensor store (box 160 rows x 16
-// bytes: 3.3 TB/s on C3's geometry against 2.0 TB/s for 16-byte STG pieces, profiles/r02_store_pieces.md).
-// Only the staging buffers are handed over (two mbarriers each, generic proxy, no fence); a helper waits for its
-// own TMA stores (bulk groups are per thread), so nobody fences or waits on the compute warps' path.  Rows
-// outside whole turns of the ring (the first 16, the last < 640) take a plain warp-level path on a
-// shared-memory copy of the ring.
+// C3 even with the stores removed).  And a CTA that holds 4 streams writes 16-byte pieces, HALF sectors: L2
+// merges the two halves of a sector only if they arrive within a few hundred clocks of each other (measured,
+// profiles/r02_store_pieces.md: 128 CTAs storing [rows x 16 bytes] boxes by TMA take 0.65 ms in lock step,
+// 1.28 ms when every second CTA runs 500 clocks late, 2.7 ms when the partners drift freely -- each lone half
+// costs a DRAM read-modify-write), which ties sector partners into lock step.  Full sectors do not care (32-byte
+// pieces: no change up to 10,000 clocks of skew).
+//
+// So: a WARP owns a stream and the recurrence shares nothing.  The window lives in registers, word i of the
+// sequence in lane i mod 32 of ring slot (i / 32) mod 20 (640 words: the window and the 16 words that complete
+// its last slot).  A step produces the 32 words of one slot, lane l from x_{i-624}, x_{i-623}, x_{i-227} --
+// lanes l+16, l+17, l+29 (mod 32) of slots k / k+1 resp. k+12 / k+13: three selects and three shuffles, no
+// shared memory, no barrier; the seven steps before a step are independent of it (227 > 7 * 32), which is the
+// instruction-level parallelism a lone warp needs.  One turn of the ring (20 steps, 640 rows) is unrolled.
+// A lone warp issues only every other clock (measured 2.1 clocks per instruction at best), so the work of a
+// number is split over two warps on the same scheduler: the COMPUTE warp of a stream runs the recurrence alone
+// (12 instructions per 32 numbers) and drops the raw words into staging columns; HELPER warps read the words of
+// a row, temper and convert them and build the row's piece in a tile of their own, which the same warp sends
+// with one TMA tensor store (bulk groups are per thread: a helper waits only for its own stores).
+// Two CTAs (8 adjacent streams) form a cluster and trade halves: rows [0, 320) of every turn are written by CTA
+// 0, rows [320, 640) by CTA 1, each for all 8 streams = full 32-byte sectors.  A compute warp writes the steps
+// that belong to its own CTA with plain shared stores and the others straight into the partner's staging
+// columns with st.async, which counts the bytes on the partner's "full" mbarrier (no fence, no flag); buffers
+// come back through "empty" mbarriers, the partner's by a remote arrive.  Nothing on the compute warps' path
+// waits for a TMA store or a proxy fence.  Rows outside whole turns of the ring (the first 16, the last < 640)
+// take a plain warp-level path on a shared-memory copy of the ring.
 constexpr int WG_S = 4;                                   // streams = compute warps = helper warps per CTA
+constexpr int WG_COLS = 2 * WG_S;                         // streams per cluster
 constexpr int WG_RING = 20;                               // ring slots (registers per lane)
 constexpr int WG_XS = 32 * WG_RING;                       // 640 words = rows per turn
-constexpr int WG_BOX = WG_XS / WG_S;                      // rows per helper and turn: one TMA box
+constexpr int WG_HALF = WG_XS / 2;                        // rows per CTA and turn
+constexpr int WG_HSTEPS = WG_RING / 2;                    // steps per CTA and turn
+constexpr int WG_BOX = WG_HALF / WG_S;                    // rows per helper and turn: one TMA box of 80 rows x 8 streams
+constexpr int WG_CP = WG_HALF + 4;                        // staging column pitch: the two CTAs' columns 16 banks apart
 constexpr int WG_NSB = 3;                                 // staging buffers
-constexpr int WG_NTB = 4;                                 // tile buffers per helper
-constexpr int WG_THREADS = 64 * WG_S;
-static_assert(WG_BOX % 32 == 0 && WG_BOX <= 256 && (WG_BOX * WG_S * 4) % 128 == 0, "bad tile");
+constexpr int WG_HW = 2 * WG_S;                           // helper warps: two per row block, taking turns
+constexpr int WG_NTB = 2;                                 // tile buffers per helper
+constexpr int WG_THREADS = 32 * (WG_S + WG_HW);
+constexpr uint32_t WG_TX = WG_HSTEPS * 32 * 4;            // bytes one partner warp sends per turn
+static_assert(WG_BOX % 16 == 0 && WG_BOX <= 256 && (WG_BOX * WG_COLS * 4) % 128 == 0 && (4 * WG_CP) % 32 == 16, "bad tile");
+
+// A waiting warp shares its scheduler with the warp it waits for: it must not spin (ncu: a bare try_wait loop took
+// 45 % of all issue slots), so it sleeps between polls.
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t a, uint32_t parity)
+{
+    for (;;) {
+        uint32_t done;
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(40);
+    }
+}
+__device__ __forceinline__ void st_async_u32(uint32_t dst_cluster, uint32_t v, uint32_t mbar_cluster)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
+                 :: "r"(dst_cluster), "r"(v), "r"(mbar_cluster) : "memory");
+}
 
 // rows [ra, rb) of one stream by its warp, ring in shared memory (word i of the call at xs[i mod 640])
 template <int DT>
@@ -1198,18 +1228,40 @@ __device__ __forceinline__ void wg_slow_rows(uint32_t *xs, uint64_t ra, uint64_t
     }
 }
 
-__device__ __forceinline__ void wg_store_row(uint32_t *p, const uint32_t (&v)[4])
+__device__ __forceinline__ void wg_store_piece(uint32_t *p, const uint32_t (&v)[4])
 {
     *reinterpret_cast<uint4 *>(p) = make_uint4(v[0], v[1], v[2], v[3]);
 }
-__device__ __forceinline__ void wg_store_row(float *p, const float (&v)[4])
+__device__ __forceinline__ void wg_store_piece(float *p, const float (&v)[4])
 {
     *reinterpret_cast<float4 *>(p) = make_float4(v[0], v[1], v[2], v[3]);
 }
-__device__ __forceinline__ void wg_store_row(double *p, const double (&v)[4])
+__device__ __forceinline__ void wg_store_piece(double *p, const double (&v)[4])
 {
     *reinterpret_cast<double2 *>(p) = make_double2(v[0], v[1]);
     *reinterpret_cast<double2 *>(p + 2) = make_double2(v[2], v[3]);
+}
+
+// One turn of the ring for the compute warp of CTA RANK: the steps of the first half of the rows belong to CTA 0,
+// the others to CTA 1; the words of the partner's steps go straight into its staging column (st.async).
+template <int RANK, int HI>
+__device__ __forceinline__ void wg_turn(uint32_t (&r)[WG_RING], uint32_t *sp, const uint32_t rp, const uint32_t rbar,
+                                        const bool ge16, const bool ge17, const bool ge29, const int l17, const int l29,
+                                        const MtMul &c)
+{
+#pragma unroll
+    for (int k = 0; k < WG_RING; k++) {                    // k = ring slot of the step (compile-time after unrolling)
+        const uint32_t v0 = ge16 ? r[k] : r[(k + 1) % WG_RING];
+        const uint32_t v1 = ge17 ? r[k] : r[(k + 1) % WG_RING];
+        const uint32_t vm = ge29 ? r[(k + 12) % WG_RING] : r[(k + 13) % WG_RING];
+        const uint32_t x0 = __shfl_xor_sync(0xffffffffu, v0, 16);
+        const uint32_t x1 = __shfl_sync(0xffffffffu, v1, l17);
+        const uint32_t xm = __shfl_sync(0xffffffffu, vm, l29);
+        const uint32_t nw = mt_recur2<HI>(x0, x1, xm, c);
+        r[k] = nw;
+        if (k / WG_HSTEPS == RANK) sp[32 * (k % WG_HSTEPS)] = nw;
+        else st_async_u32(rp + 128u * (k % WG_HSTEPS), nw, rbar);
+    }
 }
 
 template <int DT, int HI>
@@ -1219,105 +1271,107 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
 {
     typedef typename OutElem<DT>::type E;
     constexpr int W32 = (int)(sizeof(E) / 4);
-    constexpr int TILE = WG_BOX * WG_S;                   // elements per helper tile
-    // tiles [helper][NTB][TILE] of E, staging [NSB][stream][640], rings [stream][640], mbarriers sfull[NSB], sempty[NSB]
+    constexpr int TILE = WG_BOX * WG_COLS;                // elements per helper tile
+    constexpr int SBUF = WG_COLS * WG_CP;                 // words per staging buffer
+    // tiles [helper][NTB][TILE] of E, staging [NSB][8 columns][CP], rings [stream][640],
+    // mbarriers sfull[NSB], sempty[NSB], pempty[NSB]
     extern __shared__ __align__(128) uint32_t smem[];
     E *tiles = reinterpret_cast<E *>(smem);
-    uint32_t *staging = smem + WG_S * WG_NTB * TILE * W32;
-    uint32_t *rings = staging + WG_NSB * WG_S * WG_XS;
+    uint32_t *staging = smem + WG_HW * WG_NTB * TILE * W32;
+    uint32_t *rings = staging + WG_NSB * SBUF;
     const uint32_t bars = smem_addr(rings + WG_S * WG_XS);
-    const uint32_t sfull = bars, sempty = bars + 8 * WG_NSB;
+    const uint32_t sfull = bars, sempty = bars + 8 * WG_NSB, pempty = bars + 16 * WG_NSB;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint64_t s0 = (uint64_t)blockIdx.x * WG_S;
-    if (s0 >= ns) return;                                 // (the launcher guarantees ns % 4 == 0: a CTA is whole or dead)
+    uint32_t rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    const uint32_t peer = rank ^ 1u;
+    const uint64_t sc0 = (uint64_t)(blockIdx.x / 2) * WG_COLS;           // first stream of the cluster
+    const uint64_t s0 = sc0 + rank * WG_S;                                // first stream of this CTA
     if (threadIdx.x == 0) {
         for (int b = 0; b < WG_NSB; b++) {
             mbar_init(sfull + 8 * b, WG_S);
             mbar_init(sempty + 8 * b, WG_S);
+            mbar_init(pempty + 8 * b, WG_S);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
+    cluster_sync_all();                                   // both CTAs' barriers are initialised
     const uint32_t turns = n >= 16 ? (uint32_t)((n - 16) / WG_XS) : 0;   // whole turns of the ring after the first 16 rows
 
     if (warp >= WG_S) {
-        // ---- helper warp h: rows [160 h, 160 h + 160) of every turn, all four streams ----------------------
-        const int h = warp - WG_S;
-        E *my = tiles + h * WG_NTB * TILE;
+        // ---- helper warp h: rows [80 h, 80 h + 80) of this CTA's half of every turn, all eight streams -------
+        // lane = (row, half): 16 rows per pass, the even lanes take the four streams of CTA 0, the odd ones CTA 1's
+        // (helper warps h and h + 4 share the rows and alternate turns: three warps per scheduler keep it busy)
+        const int h = (warp - WG_S) % WG_S, par = (warp - WG_S) / WG_S;
+        E *my = tiles + (warp - WG_S) * WG_NTB * TILE;
         const uint32_t my_s = smem_addr(my);
-        const int x = (int)(s0 * W32);
-        for (uint32_t u = 0; u < turns; u++) {
-            const uint32_t b = u % WG_NSB, tb = u % WG_NTB;
-            if (lane == 0) {
-                mbar_wait(sfull + 8 * b, (u / WG_NSB) & 1u);
-                if (u >= WG_NTB) asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(WG_NTB - 1) : "memory");
-            }
-            __syncwarp();
-            const uint32_t *sp = staging + b * (WG_S * WG_XS) + h * WG_BOX + lane;
-            E *tp = my + tb * TILE + lane * WG_S;
+        const uint32_t peer_pempty = map_to_cta(pempty, peer);
+        const int x = (int)(sc0 * W32);
+        const int y0 = 16 + WG_HALF * (int)rank + WG_BOX * h;
+        const uint32_t *sp0 = staging + (lane & 1) * (WG_S * WG_CP) + h * WG_BOX + (lane >> 1);
+        for (uint32_t u = par; u < turns; u += 2) {
+            const uint32_t b = u % WG_NSB, tb = (u / 2) % WG_NTB;
+            // (all lanes poll and wait: no divergence to reconverge; only lane 0 has bulk groups pending)
+            mbar_wait_sleep(sfull + 8 * b, (u / WG_NSB) & 1u);
+            if (u / 2 >= WG_NTB) asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(WG_NTB - 1) : "memory");
+            const uint32_t *sp = sp0 + b * SBUF;
+            E *tp = my + tb * TILE + lane * 4;
 #pragma unroll
-            for (int i = 0; i < WG_BOX / 32; i++) {
-                E v[WG_S];
+            for (int i = 0; i < WG_BOX / 16; i++) {
+                E v[4];
 #pragma unroll
-                for (int q = 0; q < WG_S; q++) v[q] = convert<DT>(mt_temper2<HI>(sp[q * WG_XS + 32 * i], c));
-                wg_store_row(tp + 32 * i * WG_S, v);
+                for (int q = 0; q < 4; q++) v[q] = convert<DT>(mt_temper2<HI>(sp[q * WG_CP + 16 * i], c));
+                wg_store_piece(tp + 16 * i * WG_COLS, v);
             }
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // tile writes -> visible to the TMA engine
             __syncwarp();
             if (lane == 0) {
                 mbar_arrive(sempty + 8 * b);
-                tma_store_2d(&tmap, my_s + tb * (uint32_t)(TILE * sizeof(E)), x, 16 + WG_XS * (int)u + WG_BOX * h);
+                mbar_arrive_cluster(peer_pempty + 8 * b);
+                tma_store_2d(&tmap, my_s + tb * (uint32_t)(TILE * sizeof(E)), x, y0 + WG_XS * (int)u);
             }
         }
         if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-        return;
-    }
-
-    // ---- compute warp g: stream s0 + g ----------------------------------------------------------------------
-    const int g = warp;
-    uint32_t *xs = rings + g * WG_XS;
-    {
-        const uint32_t *src = st_in + (s0 + g) * NW;
-        for (int i = lane; i < NW; i += 32) xs[i] = __ldg(src + i);
-    }
-    __syncwarp();
-    E *col = out + s0 + g;
-    wg_slow_rows<DT>(xs, 0, n < 16 ? n : 16, col, ns, lane, c);
-    if (turns) {
-        uint32_t r[WG_RING];
-#pragma unroll
-        for (int q = 0; q < WG_RING; q++) r[q] = xs[32 * q + lane];
-        const bool ge16 = lane >= 16, ge17 = lane >= 17, ge29 = lane >= 29;
-        const int l17 = (lane + 17) & 31, l29 = (lane + 29) & 31;
-        for (uint32_t u = 0; u < turns; u++) {
-            const uint32_t b = u % WG_NSB;
-            if (u >= WG_NSB) {
-                if (lane == 0) mbar_wait(sempty + 8 * b, ((u / WG_NSB) - 1u) & 1u);
-                __syncwarp();
-            }
-            uint32_t *sp = staging + (b * WG_S + g) * WG_XS + lane;
-#pragma unroll
-            for (int k = 0; k < WG_RING; k++) {
-                const uint32_t v0 = ge16 ? r[k] : r[(k + 1) % WG_RING];
-                const uint32_t v1 = ge17 ? r[k] : r[(k + 1) % WG_RING];
-                const uint32_t vm = ge29 ? r[(k + 12) % WG_RING] : r[(k + 13) % WG_RING];
-                const uint32_t x0 = __shfl_xor_sync(0xffffffffu, v0, 16);
-                const uint32_t x1 = __shfl_sync(0xffffffffu, v1, l17);
-                const uint32_t xm = __shfl_sync(0xffffffffu, vm, l29);
-                const uint32_t nw = mt_recur2<HI>(x0, x1, xm, c);
-                r[k] = nw;
-                sp[32 * k] = nw;
-            }
-            __syncwarp();
-            if (lane == 0) mbar_arrive(sfull + 8 * b);
+    } else {
+        // ---- compute warp g: stream s0 + g ------------------------------------------------------------------
+        const int g = warp;
+        uint32_t *xs = rings + g * WG_XS;
+        {
+            const uint32_t *src = st_in + (s0 + g) * NW;
+            for (int i = lane; i < NW; i += 32) xs[i] = __ldg(src + i);
         }
-#pragma unroll
-        for (int q = 0; q < WG_RING; q++) xs[32 * q + lane] = r[q];
         __syncwarp();
-    }
-    wg_slow_rows<DT>(xs, n < 16 ? n : 16 + (uint64_t)turns * WG_XS, n, col, ns, lane, c);
-    // the window after n numbers: words n .. n + 623 of the call
-    {
+        E *col = out + s0 + g;
+        wg_slow_rows<DT>(xs, 0, n < 16 ? n : 16, col, ns, lane, c);
+        if (turns) {
+            uint32_t r[WG_RING];
+#pragma unroll
+            for (int q = 0; q < WG_RING; q++) r[q] = xs[32 * q + lane];
+            const bool ge16 = lane >= 16, ge17 = lane >= 17, ge29 = lane >= 29;
+            const int l17 = (lane + 17) & 31, l29 = (lane + 29) & 31;
+            // this warp's staging column (rank, g): here and in the partner CTA
+            uint32_t *lcol = staging + (rank * WG_S + g) * WG_CP + lane;
+            const uint32_t rcol = map_to_cta(smem_addr(lcol), peer);
+            const uint32_t rfull = map_to_cta(sfull, peer);
+            for (uint32_t u = 0; u < turns; u++) {
+                const uint32_t b = u % WG_NSB, ph = ((u / WG_NSB) - 1u) & 1u;
+                // both staging columns of this turn must have been read out (here by our helpers, there by the partner's)
+                if (u >= WG_NSB) {
+                    mbar_wait_sleep(sempty + 8 * b, ph);
+                    mbar_wait_sleep(pempty + 8 * b, ph);
+                }
+                if (rank == 0) wg_turn<0, HI>(r, lcol + b * SBUF, rcol + b * (uint32_t)(SBUF * 4), rfull + 8 * b, ge16, ge17, ge29, l17, l29, c);
+                else wg_turn<1, HI>(r, lcol + b * SBUF, rcol + b * (uint32_t)(SBUF * 4), rfull + 8 * b, ge16, ge17, ge29, l17, l29, c);
+                __syncwarp();
+                if (lane == 0) mbar_expect_tx(sfull + 8 * b, WG_TX);
+            }
+#pragma unroll
+            for (int q = 0; q < WG_RING; q++) xs[32 * q + lane] = r[q];
+            __syncwarp();
+        }
+        wg_slow_rows<DT>(xs, n < 16 ? n : 16 + (uint64_t)turns * WG_XS, n, col, ns, lane, c);
+        // the window after n numbers: words n .. n + 623 of the call
         uint32_t *dst = st_out + (s0 + g) * NW;
         uint32_t pos = (uint32_t)(n % WG_XS) + lane;
         for (int i = lane; i < NW; i += 32) {
@@ -1326,29 +1380,45 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
             pos += 32;
         }
     }
+    // nobody leaves while the partner may still send it words or signals
+    cluster_sync_all();
 }
+
+// the cluster kernel needs whole clusters of 8 streams on top of the TMA conditions
+bool wgen_ok(const GenArgs &a) { return a.n_streams % WG_COLS == 0 && tgen_ok(a); }
 
 template <int DT, int HI> cudaError_t launch_wgen(cudaStream_t stream, const GenArgs &a)
 {
     typedef typename OutElem<DT>::type E;
     auto kern = mt19937_wgen_kernel<DT, HI>;
-    const size_t smem = (size_t)WG_S * WG_NTB * WG_BOX * WG_S * sizeof(E) + (size_t)(WG_NSB + 1) * WG_S * WG_XS * 4 + 2 * WG_NSB * 8;
+    const size_t smem = (size_t)WG_HW * WG_NTB * WG_BOX * WG_COLS * sizeof(E) + (size_t)WG_NSB * WG_COLS * WG_CP * 4 +
+                        (size_t)WG_S * WG_XS * 4 + 3 * WG_NSB * 8;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const uint32_t w32 = (uint32_t)(sizeof(E) / 4);
     CUtensorMap tm;
     const cuuint64_t dims[2] = {a.n_streams * w32, a.n};
     const cuuint64_t strides[1] = {a.n_streams * sizeof(E)};
-    const cuuint32_t box[2] = {WG_S * w32, WG_BOX};
+    const cuuint32_t box[2] = {WG_COLS * w32, WG_BOX};
     const cuuint32_t es[2] = {1, 1};
     if (tensor_map_encoder()(&tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, a.out, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorInvalidValue;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(a.n_streams / WG_S));
+    cfg.blockDim = dim3(WG_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
     const MtMul c = {2u * 0x1908B0DFu, 1u << 31, 1u << 21, 1u << 14};
-    kern<<<(unsigned)ceil_div_u64(a.n_streams, WG_S), WG_THREADS, smem, stream>>>(
-        (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (E *)a.out, a.n_streams, a.n, c, tm);
-    return cudaGetLastError();
+    return cudaLaunchKernelEx(&cfg, kern, (const uint32_t *)a.st_in, (uint32_t *)a.st_out, (E *)a.out, a.n_streams, a.n, c, tm);
 }
 
 template <int HI> cudaError_t dispatch_wdt(cudaStream_t stream, const GenArgs &a)
@@ -1555,15 +1625,17 @@ cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *
     // prand_init refuses larger families (PRAND_MT19937_MAX_STREAMS, prand.h)
     if (a.n_streams > PRAND_MT19937_MAX_STREAMS) return cudaErrorInvalidValue;
     // Kernel choice by stream count (measured on B200): 32 streams per CTA need >= ~128
-    // CTAs; below that 8 streams per CTA; below ~1000 streams 4 per CTA in sector-sharing cluster pairs.
-    int cfg = a.n_streams >= 4096 ? 0 : a.n_streams >= 1024 ? 1 : 2;
+    // CTAs; below that 8 streams per CTA; below ~1000 streams the warp-per-stream cluster kernel if the rows are
+    // long enough to amortise its start-up (whole clusters of 8 streams, 16-byte aligned rows), else 4 streams
+    // per CTA in sector-sharing cluster pairs.
+    int cfg = a.n_streams >= 4096 ? 0 : a.n_streams >= 1024 ? 1 : (a.n >= 65536 && wgen_ok(a)) ? 6 : 2;
     // 4-byte outputs, 16-byte aligned rows: the cluster-gather kernel writes 64-byte pieces
     const bool gather_ok = a.dtype != DT_F64 && a.n_streams % 4 == 0 && (uintptr_t)a.out % 16 == 0 && a.n / NW < (1ull << 32);
     // (not the default: measured 1.29 ms on C3 against 1.00 ms for the cluster-pair kernel -- the exchange is
     // bound by the ~10-13 B/clk/SM that distributed shared memory moves between four CTAs)
     if (debug_hooks().mt_cfg >= 0) {                                          // test hook: force a variant
         const int want = debug_hooks().mt_cfg;
-        if ((want != 3 || gather_ok) && (want < 4 || tgen_ok(a))) cfg = want;
+        if ((want != 3 || gather_ok) && (want < 4 || tgen_ok(a)) && (want < 6 || wgen_ok(a))) cfg = want;
     }
     switch (cfg) {
     case 0: li->kernel = "mt19937_bgen<S=32>"; return dispatch_bdt<0>(stream, a);
@@ -1571,8 +1643,7 @@ cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *
     case 3:
         li->kernel = "mt19937_cgen<CS=4>";
         return a.dtype == DT_U32 ? launch_cgen<DT_U32>(stream, a) : launch_cgen<DT_F32>(stream, a);
-    case 6: li->kernel = "mt19937_wgen<S=4>"; return dispatch_wdt<6>(stream, a);
-    case 7: li->kernel = "mt19937_wgen<S=4>"; return dispatch_wdt<0>(stream, a);
+    case 6: li->kernel = "mt19937_wgen<CS=2>"; return dispatch_wdt<0>(stream, a);
     case 4: li->kernel = "mt19937_tgen<S=4,T=208,pair>"; return dispatch_tdt<4, 208, 1, 6, true>(stream, a);
     case 5: li->kernel = "mt19937_tgen<S=8,T=104>"; return dispatch_tdt<8, 104, 2, 0, false>(stream, a);
     default: li->kernel = "mt19937_gen<S=4,T=208,pair>"; return dispatch_dt<4, 208, 1, 6, true>(stream, a);

@@ -88,10 +88,10 @@ def test_every_output_and_state_matches_oracle(gen, dtype):
 
 MT_CFG_KERNEL = {0: "mt19937_bgen<S=32>", 1: "mt19937_gen<S=8,T=104>", 2: "mt19937_gen<S=4,T=208,pair>",
                  3: "mt19937_cgen<CS=4>", 4: "mt19937_tgen<S=4,T=208,pair>", 5: "mt19937_tgen<S=8,T=104>",
-                 6: "mt19937_wgen<S=4>", 7: "mt19937_wgen<S=4>"}
+                 6: "mt19937_wgen<CS=2>"}
 
 
-@pytest.mark.parametrize("cfg", range(8))
+@pytest.mark.parametrize("cfg", range(7))
 def test_mt19937_every_kernel_configuration(cfg, monkeypatch):
     """Every (streams per CTA, word slices, barrier interval, pipe mix, cluster pairing / cluster
     gather / TMA tile stores) variant of the MT19937 generation kernel, over whole rounds of 624, several
@@ -105,6 +105,9 @@ def test_mt19937_every_kernel_configuration(cfg, monkeypatch):
     if cfg >= 4:      # TMA tile stores: stream counts that are multiples of 4, calls of at least one round
         cases = [(4, [624, 1248, 700, 4000], "u32"), (12, [2048], "f32"), (8, [1500, 625, 3121], "f64"),
                  (68, [1300, 1872], "u32"), (36, [5000], "f32"), (20, [3000, 6240], "f64")]
+    if cfg >= 6:      # warp-per-stream cluster kernel: whole clusters of 8 streams
+        cases = [(8, [624, 1248, 700, 4000], "u32"), (16, [2048], "f32"), (8, [1500, 625, 3121], "f64"),
+                 (72, [1300, 15, 1872, 656], "u32"), (40, [5000], "f32"), (24, [3000, 6240], "f64")]
     for ns, calls, dtype in cases:
         w = Workload(f"mt-cfg{cfg}", "mt19937", 5489, ns, 1000, sum(calls), dtype)
         got, st, kernel = lib_run(w, calls=calls)
@@ -346,14 +349,14 @@ def test_mt19937_every_polynomial_application_kernel(hook):
         assert st[s * sb:(s + 1) * sb] == wst.tobytes(), (hook, s)
 
 
-@pytest.mark.parametrize("cfg", range(8))
+@pytest.mark.parametrize("cfg", range(7))
 def test_shared_memory_kernels_repeat_bit_for_bit(cfg):
     """compute-sanitizer is not available on this GPU pool, so races in the shared-memory MT19937 kernels (in-place
     circular windows, deferred tempering, split cluster barriers, cp.async state loads, DSMEM bulk copies) are hunted
     by repetition instead: every kernel variant runs eight times from the same state at a size that fills the GPU,
     and all runs must agree bit for bit with the first, which is checked against the oracle on sampled streams."""
     need_gpu()
-    ns = {0: 4736, 1: 1184, 2: 592, 3: 592, 4: 592, 5: 1184, 6: 592, 7: 592}[cfg]   # 148 CTAs of 32 / 8 / 4 / 4 / 4 / 8 streams
+    ns = {0: 4736, 1: 1184, 2: 592, 3: 592, 4: 592, 5: 1184, 6: 592}[cfg]   # 148 CTAs of 32 / 8 / 4 / 4 / 4 / 8 streams
     n = 624 * 9 + 77
     P.prand_debug_set("PRAND_MT_CFG", str(cfg))
     try:
