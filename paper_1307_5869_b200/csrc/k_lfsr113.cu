@@ -286,7 +286,8 @@ cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
 template <int DT> cudaError_t dispatch_v(cudaStream_t stream, const GenArgs &a, LaunchInfo *li)
 {
     // 128-bit stores need 4 adjacent streams per thread and 16-byte aligned rows.
-    bool vec = (a.n_streams % 4 == 0) && ((uintptr_t)a.out % 16 == 0) && ((uintptr_t)a.st_in % 16 == 0);
+    bool vec = (a.n_streams % 4 == 0) && ((uintptr_t)a.out % 16 == 0) && ((uintptr_t)a.st_in % 16 == 0) &&
+               !lfsr113_narrow(a.n_streams, a.n, a.dtype, sm_count());
     li->launches = 1;
     if (vec) { li->kernel = "lfsr113_gen<V=4>"; return launch_gen<4, DT>(stream, a); }
     li->kernel = "lfsr113_gen<V=1>";

@@ -54,6 +54,56 @@ mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
                                                (int)(blockIdx.x % SPLIT) * NOUT);
 }
 
+// Latency form of the same application (a handful of destination streams: the first levels of a doubling tree,
+// where a level lasts as long as ONE application and 140 SMs idle).  An application is cut into 39 CTAs of 16
+// output words; every CTA extends the window itself (88 rounds of 227 words, 4.5 us) and thread (word j, slice s)
+// of its 256 threads XORs the words selected by the polynomial words s, s + 16, ...: 39 coefficient words per
+// thread, scanned bit by bit two words at a time (two independent chains), then the 16 slices of a word are
+// folded through shared memory.  ~15 us per level against ~90 us for the 4-CTA split.  src != dst only.
+constexpr int AW_OUT = 16, AW_SL = 16, AW_THREADS = AW_OUT * AW_SL, AW_PARTS = NW / AW_OUT;
+
+__global__ void __launch_bounds__(AW_THREADS)
+mt19937_apply_wide_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0, uint64_t src_back,
+                          const MtOp *__restrict__ op)
+{
+    extern __shared__ __align__(16) uint32_t smem[];
+    uint32_t *x = smem;                                    // APPLY_XWORDS, then AW_SL * AW_OUT partial sums
+    uint32_t *red = smem + APPLY_XWORDS + 3;
+    const int tid = threadIdx.x;
+    const uint64_t dst = dst0 + blockIdx.x / AW_PARTS;
+    const int out0 = (int)(blockIdx.x % AW_PARTS) * AW_OUT;
+    const uint32_t *src = st_src + (dst - src_back) * NW;
+    for (int j = tid; j < NW; j += AW_THREADS) x[j] = src[j];
+    __syncthreads();
+    for (int r0 = 0; r0 < DEG; r0 += NW - MW) {
+        const int k = r0 + tid;
+        if (tid < NW - MW && k < DEG) x[NW + k] = mt_recur(x[k], x[k + 1], x[k + MW]);
+        __syncthreads();
+    }
+    const int j = tid % AW_OUT, sl = tid / AW_OUT;
+    const uint32_t *xo = x + out0 + j;
+    uint32_t acc0 = 0, acc1 = 0;
+    for (int wi = sl; wi < NW; wi += 2 * AW_SL) {
+        uint32_t p0 = __ldg(&op->w[wi]);
+        uint32_t p1 = wi + AW_SL < NW ? __ldg(&op->w[wi + AW_SL]) : 0u;
+        const uint32_t *x0 = xo + 32 * wi, *x1 = x0 + 32 * AW_SL;
+        while (p0 | p1) {                                  // (uniform within the 16 threads of a slice)
+            if (p0) { acc0 ^= x0[__ffs(p0) - 1]; p0 &= p0 - 1; }
+            if (p1) { acc1 ^= x1[__ffs(p1) - 1]; p1 &= p1 - 1; }
+        }
+    }
+    red[sl * AW_OUT + j] = acc0 ^ acc1;
+    __syncthreads();
+    if (tid < AW_OUT) {
+        uint32_t a = 0;
+#pragma unroll
+        for (int q = 0; q < AW_SL; q++) a ^= red[q * AW_OUT + tid];
+        const int w = out0 + tid;
+        st_dst[dst * NW + w] = w == 0 ? (a & 0x80000000u) : a;   // only the top bit of word 0 is state (T2)
+    }
+}
+constexpr size_t AW_SMEM = (size_t)(APPLY_XWORDS + 3 + AW_SL * AW_OUT) * sizeof(uint32_t);
+
 // Throughput form of the same application (many destination streams).  Thread t accumulates the four
 // consecutive output words 4t .. 4t+3.  For the 32 coefficients of one polynomial word pw (positions
 // 32 wi + b) they read x[32 wi + 4t + b + c], c < 4: a window of 35 consecutive words, loaded as nine
@@ -1585,8 +1635,14 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
     li->launches = 0;
     // grid.x is limited to 2^31-1 blocks; streams beyond that would not fit device memory anyway
     if (count == 0) return cudaSuccess;
+    // a handful of applications: the launch is as long as one application, spread each over 39 CTAs
+    if (src_back != 0 && !debug_hooks().mt_apply_list && !debug_hooks().mt_apply_win && count * AW_PARTS <= 4 * (uint64_t)sm_count()) {
+        e = cudaFuncSetAttribute(mt19937_apply_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AW_SMEM);
+        if (e != cudaSuccess) return e;
+        mt19937_apply_wide_kernel<<<(unsigned)(count * AW_PARTS), AW_THREADS, AW_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+    }
     // fewer CTAs than SMs: the launch is as long as one application
-    if (src_back != 0 && 4 * count <= 2 * (uint64_t)sm_count())
+    else if (src_back != 0 && 4 * count <= 2 * (uint64_t)sm_count())
         mt19937_apply_kernel<160, 4><<<(unsigned)(4 * count), 160, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     else if (count <= (uint64_t)sm_count())
         mt19937_apply_kernel<640, 1><<<(unsigned)count, 640, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);

@@ -594,7 +594,7 @@ void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t 
     } else {
         // threads one launch gets without chunking
         uint64_t per_thread_streams = 1, lanes_per_stream = 1, min_len = 64;
-        if (gen == PRAND_LFSR113) per_thread_streams = 4;
+        if (gen == PRAND_LFSR113) per_thread_streams = lfsr113_narrow(ns, n, dtype, sms) ? 1 : 4;
         else if (gen == PRAND_MRG32K3A) per_thread_streams = dtype == DT_F64 ? 2 : 4;
         else {
             min_len = 128;

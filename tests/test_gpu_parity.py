@@ -329,8 +329,9 @@ def test_set_state_refuses_words_the_kernels_cannot_take():
 def test_mt19937_every_polynomial_application_kernel(hook):
     """Eq. 10 in all its kernels: the four-streams-per-CTA form with the polynomial as a
     kernel argument (tree levels of >= 2368 streams) and from device memory (prand_jump by a distance that is
-    not tabulated), the one-stream window form and the position-list form (hooks), the 640-thread and the
-    4-CTA split forms of the small levels.  Sampled streams against the oracle."""
+    not tabulated), the one-stream window form and the position-list form (hooks), the 39-CTA wide form of the
+    first levels (no hook) and the 640-thread and 4-CTA split forms that take its place under the hooks.
+    Sampled streams against the oracle."""
     need_gpu()
     ns, L, steps = 6000, 2**64, (2**40 + 12345) << 480
     P.prand_debug_set("PRAND_MT_APPLY", hook)
@@ -343,7 +344,7 @@ def test_mt19937_every_polynomial_application_kernel(hook):
     finally:
         P.prand_debug_set("PRAND_MT_APPLY", None)
     sb = oracle.state_bytes("mt19937")
-    for s in (0, 2047, 2048, 4096, ns - 1):
+    for s in (0, 1, 3, 6, 13, 2047, 2048, 4096, ns - 1):
         want, wst = oracle.streams("mt19937", 5489, s, 1, L, 40, "u32", pre_jump=steps)
         assert np.array_equal(got[:, s], want[:, 0]), (hook, s)
         assert st[s * sb:(s + 1) * sb] == wst.tobytes(), (hook, s)
