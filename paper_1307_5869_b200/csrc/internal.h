@@ -113,7 +113,9 @@ int sm_count();   // multiprocessor count of the current device
 struct DebugHooks {
     int mt_cfg;             // PRAND_MT_CFG: force an MT19937 generation kernel variant (-1: by stream count)
     bool mt_apply_list;     // PRAND_MT_APPLY=list: the position-list application kernel at any size
-    bool mt_apply_win;      // PRAND_MT_APPLY=win: the one-stream-per-CTA window kernel instead of four streams per CTA
+    bool mt_apply_win;      // PRAND_MT_APPLY=win | win2 | win4: the one-stream-per-CTA window kernel (1, 2 or 4 slices of
+                            // 160 threads) at any size, instead of the forms chosen by the number of applications
+    int mt_apply_nsl;
     int gm_lp;              // PRAND_GM_LP: lanes per GM61 stream (0: default)
     int gm31_nf;            // PRAND_GM31_NF: GM31 points on the FP64 pipe (-1: default 14)
     bool gm_watch_set;      // PRAND_GM_WATCH: limit of the optimistic steps' watch value

@@ -58,8 +58,8 @@ mt19937_apply_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
 // where a level lasts as long as ONE application and 140 SMs idle).  An application is cut into 39 CTAs of 16
 // output words; every CTA extends the window itself (88 rounds of 227 words, 4.5 us) and thread (word j, slice s)
 // of its 256 threads XORs the words selected by the polynomial words s, s + 16, ...: 39 coefficient words per
-// thread, scanned bit by bit two words at a time (two independent chains), then the 16 slices of a word are
-// folded through shared memory.  ~15 us per level against ~90 us for the 4-CTA split.  src != dst only.
+// thread, every coefficient visited branch-free (a bit scan was latency-bound: 58 us), then the 16 slices of a
+// word are folded through shared memory.  src != dst only.
 constexpr int AW_OUT = 16, AW_SL = 16, AW_THREADS = AW_OUT * AW_SL, AW_PARTS = NW / AW_OUT;
 
 __global__ void __launch_bounds__(AW_THREADS)
@@ -82,14 +82,17 @@ mt19937_apply_wide_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst
     }
     const int j = tid % AW_OUT, sl = tid / AW_OUT;
     const uint32_t *xo = x + out0 + j;
+    // no bit scan, no branch: every coefficient is visited, its word loaded at a compile-time offset and masked
+    // (a load and two logic operations per coefficient, all independent: the loop runs at issue rate)
     uint32_t acc0 = 0, acc1 = 0;
-    for (int wi = sl; wi < NW; wi += 2 * AW_SL) {
-        uint32_t p0 = __ldg(&op->w[wi]);
-        uint32_t p1 = wi + AW_SL < NW ? __ldg(&op->w[wi + AW_SL]) : 0u;
-        const uint32_t *x0 = xo + 32 * wi, *x1 = x0 + 32 * AW_SL;
-        while (p0 | p1) {                                  // (uniform within the 16 threads of a slice)
-            if (p0) { acc0 ^= x0[__ffs(p0) - 1]; p0 &= p0 - 1; }
-            if (p1) { acc1 ^= x1[__ffs(p1) - 1]; p1 &= p1 - 1; }
+#pragma unroll 1
+    for (int wi = sl; wi < NW; wi += AW_SL) {
+        const uint32_t pw = __ldg(&op->w[wi]);
+        const uint32_t *xw = xo + 32 * wi;
+#pragma unroll
+        for (int b = 0; b < 32; b += 2) {
+            acc0 ^= xw[b] & (uint32_t)((int32_t)(pw << (31 - b)) >> 31);
+            acc1 ^= xw[b + 1] & (uint32_t)((int32_t)(pw << (30 - b)) >> 31);
         }
     }
     red[sl * AW_OUT + j] = acc0 ^ acc1;
@@ -111,61 +114,84 @@ constexpr size_t AW_SMEM = (size_t)(APPLY_XWORDS + 3 + AW_SL * AW_OUT) * sizeof(
 // four register XORs.  36 words loaded per 64 XORs on average instead of one load per XOR.
 constexpr int APPLYW_THREADS = 160;                         // 156 active in the accumulation
 
-__global__ void __launch_bounds__(APPLYW_THREADS)
+// NSL > 1: the coefficient words are dealt to NSL slices of 160 threads whose partial sums are folded through
+// shared memory -- the same work in 1 / NSL of the time for launches of a few hundred applications, where a
+// level of the tree lasts as long as one CTA (NSL = 4: one CTA per SM, NSL = 2: two).
+template <int NSL>
+__global__ void __launch_bounds__(APPLYW_THREADS * NSL)
 mt19937_apply_win_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t dst0,
                          uint64_t src_back, const MtOp *__restrict__ op)
 {
+    constexpr int NT = APPLYW_THREADS * NSL;
+    constexpr int EXT = NT < NW - MW ? NT : NW - MW;       // at most 227 new words are independent
+    static_assert((NW / 2) % NSL == 0, "the slices take whole pairs of coefficient words");
     extern __shared__ __align__(16) uint32_t smem[];
-    uint32_t *x = smem;                                    // APPLY_XWORDS + APPLY_ZPAD
+    uint32_t *x = smem;                                    // APPLY_XWORDS + APPLY_ZPAD, then [NSL][624] partial sums
+    uint32_t *red = smem + (APPLY_XWORDS + APPLY_ZPAD + 3) / 4 * 4;
     const int tid = threadIdx.x;
     const uint64_t dst = dst0 + blockIdx.x;
     const uint32_t *src = st_src + (dst - src_back) * NW;
-    for (int j = tid; j < NW; j += APPLYW_THREADS) x[j] = src[j];
-    for (int j = tid; j < APPLY_ZPAD; j += APPLYW_THREADS) x[APPLY_ZERO + j] = 0;
+    for (int j = tid; j < NW; j += NT) x[j] = src[j];
+    for (int j = tid; j < APPLY_ZPAD; j += NT) x[APPLY_ZERO + j] = 0;
     __syncthreads();
-    for (int r0 = 0; r0 < DEG; r0 += APPLYW_THREADS) {
+    for (int r0 = 0; r0 < DEG; r0 += EXT) {
         int k = r0 + tid;
-        if (k < DEG) x[NW + k] = mt_recur(x[k], x[k + 1], x[k + MW]);
+        if (tid < EXT && k < DEG) x[NW + k] = mt_recur(x[k], x[k + 1], x[k + MW]);
         __syncthreads();
     }
-    if (tid >= NW / 4) return;
-    uint32_t acc[4][4] = {};                               // four interleaved sets: independent XOR chains
-    const uint4 *xw = reinterpret_cast<const uint4 *>(x) + tid;   // window of wi starts at xw[8 wi]
-    // two register windows in ping-pong: the nine loads of the next polynomial word are issued before
-    // the 128 predicated XORs of the current one
-    uint4 wa[9], wb[9];
-    auto load_win = [&](uint4 (&w)[9], int wi) {
+    const int q = tid / APPLYW_THREADS, t = tid % APPLYW_THREADS;
+    const bool accum = t < NW / 4;
+    uint32_t r[4] = {0u, 0u, 0u, 0u};
+    if (accum) {
+        uint32_t acc[4][4] = {};                           // four interleaved sets: independent XOR chains
+        const uint4 *xw = reinterpret_cast<const uint4 *>(x) + t;     // window of wi starts at xw[8 wi]
+        // two register windows in ping-pong: the nine loads of the next polynomial word are issued before
+        // the 128 predicated XORs of the current one
+        uint4 wa[9], wb[9];
+        auto load_win = [&](uint4 (&w)[9], int wi) {
 #pragma unroll
-        for (int q = 0; q < 9; q++) w[q] = xw[8 * wi + q];
-    };
-    auto accumulate = [&](const uint4 (&w)[9], uint32_t pw) {
-        uint32_t v[36];
+            for (int m = 0; m < 9; m++) w[m] = xw[8 * wi + m];
+        };
+        auto accumulate = [&](const uint4 (&w)[9], uint32_t pw) {
+            uint32_t v[36];
 #pragma unroll
-        for (int q = 0; q < 9; q++) { v[4 * q] = w[q].x; v[4 * q + 1] = w[q].y; v[4 * q + 2] = w[q].z; v[4 * q + 3] = w[q].w; }
+            for (int m = 0; m < 9; m++) { v[4 * m] = w[m].x; v[4 * m + 1] = w[m].y; v[4 * m + 2] = w[m].z; v[4 * m + 3] = w[m].w; }
 #pragma unroll
-        for (int b = 0; b < 32; b++) {
-            if (pw & (1u << b)) {
-                acc[b & 3][0] ^= v[b]; acc[b & 3][1] ^= v[b + 1]; acc[b & 3][2] ^= v[b + 2]; acc[b & 3][3] ^= v[b + 3];
+            for (int b = 0; b < 32; b++) {
+                if (pw & (1u << b)) {
+                    acc[b & 3][0] ^= v[b]; acc[b & 3][1] ^= v[b + 1]; acc[b & 3][2] ^= v[b + 2]; acc[b & 3][3] ^= v[b + 3];
+                }
             }
-        }
-    };
-    load_win(wa, 0);
-    uint32_t pw0 = __ldg(&op->w[0]), pw1 = __ldg(&op->w[1]);
+        };
+        constexpr int STEP = 2 * NSL;                      // slice q takes the word pairs 2q, 2q + 2 NSL, ...
+        load_win(wa, 2 * q);
+        uint32_t pw0 = __ldg(&op->w[2 * q]), pw1 = __ldg(&op->w[2 * q + 1]);
 #pragma unroll 1
-    for (int wi = 0; wi < NW; wi += 2) {
-        load_win(wb, wi + 1);
-        const uint32_t p0 = pw0, p1 = pw1;
-        if (wi + 2 < NW) { pw0 = __ldg(&op->w[wi + 2]); pw1 = __ldg(&op->w[wi + 3]); }
-        accumulate(wa, p0);
-        load_win(wa, wi + 2 < NW ? wi + 2 : wi);
-        accumulate(wb, p1);
-    }
-    uint32_t *d = st_dst + dst * NW + 4 * tid;
-    uint32_t r[4];
+        for (int wi = 2 * q; wi < NW; wi += STEP) {
+            load_win(wb, wi + 1);
+            const uint32_t p0 = pw0, p1 = pw1;
+            if (wi + STEP < NW) { pw0 = __ldg(&op->w[wi + STEP]); pw1 = __ldg(&op->w[wi + STEP + 1]); }
+            accumulate(wa, p0);
+            load_win(wa, wi + STEP < NW ? wi + STEP : wi);
+            accumulate(wb, p1);
+        }
 #pragma unroll
-    for (int c = 0; c < 4; c++) r[c] = acc[0][c] ^ acc[1][c] ^ acc[2][c] ^ acc[3][c];
-    *reinterpret_cast<uint4 *>(d) = make_uint4(tid == 0 ? (r[0] & 0x80000000u) : r[0], r[1], r[2], r[3]);
+        for (int c = 0; c < 4; c++) r[c] = acc[0][c] ^ acc[1][c] ^ acc[2][c] ^ acc[3][c];
+    }
+    if (NSL > 1) {
+        if (accum) *reinterpret_cast<uint4 *>(red + q * NW + 4 * t) = make_uint4(r[0], r[1], r[2], r[3]);
+        __syncthreads();
+        if (q != 0 || !accum) return;
+#pragma unroll
+        for (int o = 1; o < NSL; o++) {
+            const uint4 v = *reinterpret_cast<const uint4 *>(red + o * NW + 4 * t);
+            r[0] ^= v.x; r[1] ^= v.y; r[2] ^= v.z; r[3] ^= v.w;
+        }
+    } else if (!accum) return;
+    uint32_t *d = st_dst + dst * NW + 4 * t;
+    *reinterpret_cast<uint4 *>(d) = make_uint4(t == 0 ? (r[0] & 0x80000000u) : r[0], r[1], r[2], r[3]);
 }
+template <int NSL> constexpr size_t applyw_smem() { return ((APPLY_XWORDS + APPLY_ZPAD + 3) / 4 * 4 + (NSL > 1 ? NSL * NW : 0)) * sizeof(uint32_t); }
 
 // Many destination streams, second form: FOUR streams per CTA share the control flow.  The coefficient word
 // is the same for every thread and every stream, so its bits are consumed two at a time through warp-uniform
@@ -1629,31 +1655,45 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
     if (e == cudaSuccess)
         e = cudaFuncSetAttribute(mt19937_apply_kernel<160, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)APPLY_SMEM);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(mt19937_apply_win_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)APPLY_SMEM);
+        e = cudaFuncSetAttribute(mt19937_apply_win_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)applyw_smem<1>());
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(mt19937_apply_win_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)applyw_smem<2>());
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(mt19937_apply_win_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)applyw_smem<4>());
     if (e != cudaSuccess) return e;
     li->kernel = "mt19937_apply";
     li->launches = 0;
     // grid.x is limited to 2^31-1 blocks; streams beyond that would not fit device memory anyway
     if (count == 0) return cudaSuccess;
-    // a handful of applications: the launch is as long as one application, spread each over 39 CTAs
-    if (src_back != 0 && !debug_hooks().mt_apply_list && !debug_hooks().mt_apply_win && count * AW_PARTS <= 4 * (uint64_t)sm_count()) {
+    const uint64_t sms = (uint64_t)sm_count();
+    const DebugHooks &hk = debug_hooks();
+    auto win = [&](int nsl) {
+        if (nsl == 4) mt19937_apply_win_kernel<4><<<(unsigned)count, 4 * APPLYW_THREADS, applyw_smem<4>(), stream>>>(st_src, st_dst, dst0, src_back, d_op);
+        else if (nsl == 2) mt19937_apply_win_kernel<2><<<(unsigned)count, 2 * APPLYW_THREADS, applyw_smem<2>(), stream>>>(st_src, st_dst, dst0, src_back, d_op);
+        else mt19937_apply_win_kernel<1><<<(unsigned)count, APPLYW_THREADS, applyw_smem<1>(), stream>>>(st_src, st_dst, dst0, src_back, d_op);
+    };
+    if (hk.mt_apply_list) {                                  // test hook: the position-list kernels
+        if (src_back != 0 && 4 * count <= 2 * sms)
+            mt19937_apply_kernel<160, 4><<<(unsigned)(4 * count), 160, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+        else if (count <= sms)
+            mt19937_apply_kernel<640, 1><<<(unsigned)count, 640, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+        else
+            mt19937_apply_kernel<256, 1><<<(unsigned)count, 256, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
+    } else if (hk.mt_apply_win) {                            // test hook: a window kernel at any size
+        win(hk.mt_apply_nsl);
+    } else if (src_back != 0 && count * AW_PARTS <= 5 * sms) {
+        // a handful of applications: the launch is as long as one application, spread each over 39 CTAs
         e = cudaFuncSetAttribute(mt19937_apply_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AW_SMEM);
         if (e != cudaSuccess) return e;
         mt19937_apply_wide_kernel<<<(unsigned)(count * AW_PARTS), AW_THREADS, AW_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    }
-    // fewer CTAs than SMs: the launch is as long as one application
-    else if (src_back != 0 && 4 * count <= 2 * (uint64_t)sm_count())
-        mt19937_apply_kernel<160, 4><<<(unsigned)(4 * count), 160, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    else if (count <= (uint64_t)sm_count())
-        mt19937_apply_kernel<640, 1><<<(unsigned)count, 640, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    else if (debug_hooks().mt_apply_list)                    // test hook: the position-list kernel at any size
-        mt19937_apply_kernel<256, 1><<<(unsigned)count, 256, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    else if (debug_hooks().mt_apply_win || count < 16 * (uint64_t)sm_count())   // (or the test hook) one stream per CTA
-        mt19937_apply_win_kernel<<<(unsigned)count, APPLYW_THREADS, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    else if (h_op)
+    } else if (count < 16 * sms) {
+        // up to a few thousand applications a level lasts as long as a CTA: four slices per CTA (measured: 148
+        // applications 0.127 ms against 0.203 ms with one slice and 0.162 ms for the position list, 1024: 0.85 / 0.95 / 1.07)
+        win(4);
+    } else if (h_op) {
         mt19937_apply_multi_kernel<true><<<(unsigned)ceil_div_u64(count, AM_S), AM_THREADS, 0, stream>>>(
             st_src, st_dst, dst0, count, src_back, d_op, *h_op);
-    else {
+    } else {
         static const MtOp none = {};
         mt19937_apply_multi_kernel<false><<<(unsigned)ceil_div_u64(count, AM_S), AM_THREADS, 0, stream>>>(
             st_src, st_dst, dst0, count, src_back, d_op, none);

@@ -64,7 +64,12 @@ void hook_assign(DebugHooks &h, const std::string &name, const char *v)
 {
     const bool on = v && *v;
     if (name == "PRAND_MT_CFG") h.mt_cfg = on ? std::atoi(v) : -1;
-    else if (name == "PRAND_MT_APPLY") { h.mt_apply_list = on && std::string(v) == "list"; h.mt_apply_win = on && std::string(v) == "win"; }
+    else if (name == "PRAND_MT_APPLY") {
+        const std::string m = on ? v : "";
+        h.mt_apply_list = m == "list";
+        h.mt_apply_nsl = m == "win" ? 1 : m == "win2" ? 2 : m == "win4" ? 4 : 0;
+        h.mt_apply_win = h.mt_apply_nsl != 0;
+    }
     else if (name == "PRAND_GM_LP") h.gm_lp = on ? std::atoi(v) : 0;
     else if (name == "PRAND_GM31_NF") h.gm31_nf = on ? std::atoi(v) : -1;
     else if (name == "PRAND_GM_WATCH") { h.gm_watch_set = on; h.gm_watch = on ? (uint32_t)std::strtoul(v, nullptr, 0) : 0; }

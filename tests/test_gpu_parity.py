@@ -325,12 +325,13 @@ def test_set_state_refuses_words_the_kernels_cannot_take():
     assert P.lib().prand_trim() == 0
 
 
-@pytest.mark.parametrize("hook", [None, "win", "list"])
+@pytest.mark.parametrize("hook", [None, "win", "win2", "win4", "list"])
 def test_mt19937_every_polynomial_application_kernel(hook):
     """Eq. 10 in all its kernels: the four-streams-per-CTA form with the polynomial as a
     kernel argument (tree levels of >= 2368 streams) and from device memory (prand_jump by a distance that is
-    not tabulated), the one-stream window form and the position-list form (hooks), the 39-CTA wide form of the
-    first levels (no hook) and the 640-thread and 4-CTA split forms that take its place under the hooks.
+    not tabulated), the one-stream window form with one, two and four slices and the position-list forms (hooks),
+    the 39-CTA wide form of the first levels (no hook) and the 640-thread and 4-CTA split forms that take its place
+    under the "list" hook.
     Sampled streams against the oracle."""
     need_gpu()
     ns, L, steps = 6000, 2**64, (2**40 + 12345) << 480
