@@ -233,6 +233,45 @@ mt19937_apply_multi_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t ds
     __syncthreads();
     const bool accum = tid < NW / 4;
     uint32_t acc[AM_S][4] = {};
+    // The window of a piece (AM_WB = 8 coefficients: words 4 tid + h .. + 11 of each stream) slides by 8 words from
+    // one piece to the next, so 4 of its 12 words are the last 4 of the previous piece's: the windows are a ring of
+    // four 4-word groups per stream and a piece loads only TWO new groups (two 16-byte shared loads per stream
+    // instead of three) -- shared-memory bandwidth is what bounds this kernel (ncu: L1TEX 88 %, ALU pipe 62 %).
+    // Two pieces are unrolled so that the groups rotate by renaming: piece A uses groups (0, 1, 2), piece B (2, 3, 0).
+    uint32_t G[AM_S][4][4];
+    auto load_group = [&](int g, int pos) {                // group g <- words pos .. pos + 3 (pos = 0 mod 4)
+#pragma unroll
+        for (int q = 0; q < AM_S; q++) {
+            const uint4 t = *reinterpret_cast<const uint4 *>(&ring[q][pos & (AM_RING - 1)]);
+            G[q][g][0] = t.x; G[q][g][1] = t.y; G[q][g][2] = t.z; G[q][g][3] = t.w;
+        }
+    };
+    auto piece = [&](uint32_t ph, int g0, int g1, int g2) {   // window word i = group (g0, g1, g2)[i / 4], word i % 4
+        auto W = [&](int q, int i) -> uint32_t { return G[q][i < 4 ? g0 : i < 8 ? g1 : g2][i & 3]; };
+#pragma unroll
+        for (int b = 0; b < AM_WB; b += 2) {
+            const bool lo = ph & (1u << b), hi = ph & (2u << b);     // warp-uniform
+            if (lo) {
+                if (hi) {
+#pragma unroll
+                    for (int q = 0; q < AM_S; q++)
+#pragma unroll
+                        for (int o = 0; o < 4; o++) acc[q][o] = xor3(acc[q][o], W(q, b + o), W(q, b + 1 + o));
+                } else {
+#pragma unroll
+                    for (int q = 0; q < AM_S; q++)
+#pragma unroll
+                        for (int o = 0; o < 4; o++) acc[q][o] ^= W(q, b + o);
+                }
+            } else if (hi) {
+#pragma unroll
+                for (int q = 0; q < AM_S; q++)
+#pragma unroll
+                    for (int o = 0; o < 4; o++) acc[q][o] ^= W(q, b + 1 + o);
+            }
+        }
+    };
+    if (accum) load_group(0, 4 * tid);                     // the first piece's first group
     uint32_t pw = PARAM ? 0u : __ldg(&op->w[0]);
 #pragma unroll 1
     for (int wi = 0; wi < NW; wi++) {
@@ -240,42 +279,17 @@ mt19937_apply_multi_kernel(const uint32_t *st_src, uint32_t *st_dst, uint64_t ds
         if (!PARAM && wi + 1 < NW) pw = __ldg(&op->w[wi + 1]);
         generate(32 * wi + 32);                            // x_{32 wi + 656} .. : the words step wi + 1 adds to the windows
         if (accum) {
-            // the word's 32 coefficients in AM_WB-bit pieces: a window of AM_WB + 3 (rounded to 4) words per stream
-            // (short windows keep 4 x 4 accumulators + 4 windows at 80 registers: four CTAs per SM, and the piece's
-            // code is executed four times per word instead of being unrolled: 15 KB of instructions)
+            // the word's 32 coefficients in four pieces of AM_WB (the code of two pieces is executed twice per word
+            // instead of being unrolled further)
 #pragma unroll 1
-            for (int h = 0; h < 32; h += AM_WB) {
-                uint32_t v[AM_S][AM_WB + 4];
-#pragma unroll
-                for (int q = 0; q < AM_S; q++)
-#pragma unroll
-                    for (int m = 0; m < (AM_WB + 4) / 4; m++) {
-                        const uint4 t = *reinterpret_cast<const uint4 *>(&ring[q][(32 * wi + h + 4 * tid + 4 * m) & (AM_RING - 1)]);
-                        v[q][4 * m] = t.x; v[q][4 * m + 1] = t.y; v[q][4 * m + 2] = t.z; v[q][4 * m + 3] = t.w;
-                    }
-                const uint32_t ph = p >> h;
-#pragma unroll
-                for (int b = 0; b < AM_WB; b += 2) {
-                    const bool lo = ph & (1u << b), hi = ph & (2u << b);     // warp-uniform
-                    if (lo) {
-                        if (hi) {
-#pragma unroll
-                            for (int q = 0; q < AM_S; q++)
-#pragma unroll
-                                for (int o = 0; o < 4; o++) acc[q][o] = xor3(acc[q][o], v[q][b + o], v[q][b + 1 + o]);
-                        } else {
-#pragma unroll
-                            for (int q = 0; q < AM_S; q++)
-#pragma unroll
-                                for (int o = 0; o < 4; o++) acc[q][o] ^= v[q][b + o];
-                        }
-                    } else if (hi) {
-#pragma unroll
-                        for (int q = 0; q < AM_S; q++)
-#pragma unroll
-                            for (int o = 0; o < 4; o++) acc[q][o] ^= v[q][b + 1 + o];
-                    }
-                }
+            for (int h = 0; h < 32; h += 2 * AM_WB) {
+                const int pos = 32 * wi + h + 4 * tid;
+                load_group(1, pos + 4);
+                load_group(2, pos + 8);
+                piece(p >> h, 0, 1, 2);
+                load_group(3, pos + 12);
+                load_group(0, pos + 16);                   // (the last one of a word is the next word's first group)
+                piece(p >> (h + AM_WB), 2, 3, 0);
             }
         }
         __syncthreads();
