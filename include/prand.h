@@ -271,7 +271,7 @@ int prand_probe_store_pieces(void *d_buf, size_t buf_bytes, int method, int piec
  *   change.  The hooks live in one process-wide table that is filled once from the environment
  *   variables of the same names when the library first needs it; this call changes one entry afterwards
  *   (value NULL or "" restores the default).  Names: PRAND_MT_CFG (0..6: MT19937 generation kernel),
- *   PRAND_MT_APPLY (list, win, win2, win4: other polynomial-application kernels), PRAND_GM_LP (1, 2, 4), PRAND_GM31_NF (0, 10, 12, 14, 16), PRAND_GM_WATCH,
+ *   PRAND_MT_APPLY (list, win, win2, win4, multi: other polynomial-application kernels), PRAND_GM_LP (1, 2, 4), PRAND_GM31_NF (0, 10, 12, 14, 16), PRAND_GM_WATCH,
  *   PRAND_MRG_INT, PRAND_GM_INIT (matrix), PRAND_CHUNK_LEN, PRAND_LFSR_INIT (table: the paper's 128-table
  *   jump), PRAND_MT_POLY (host: no precomputed polynomial table).  Unknown name:
  *   PRAND_ERR_ARG.

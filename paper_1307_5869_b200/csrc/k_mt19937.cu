@@ -1695,14 +1695,15 @@ cudaError_t mt19937_apply(cudaStream_t stream, const uint32_t *st_src, uint32_t 
             mt19937_apply_kernel<256, 1><<<(unsigned)count, 256, APPLY_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
     } else if (hk.mt_apply_win) {                            // test hook: a window kernel at any size
         win(hk.mt_apply_nsl);
-    } else if (src_back != 0 && count * AW_PARTS <= 5 * sms) {
+    } else if (hk.mt_apply_nsl >= 0 && src_back != 0 && count * AW_PARTS <= 5 * sms) {
         // a handful of applications: the launch is as long as one application, spread each over 39 CTAs
         e = cudaFuncSetAttribute(mt19937_apply_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AW_SMEM);
         if (e != cudaSuccess) return e;
         mt19937_apply_wide_kernel<<<(unsigned)(count * AW_PARTS), AW_THREADS, AW_SMEM, stream>>>(st_src, st_dst, dst0, src_back, d_op);
-    } else if (count < 16 * sms) {
-        // up to a few thousand applications a level lasts as long as a CTA: four slices per CTA (measured: 148
-        // applications 0.127 ms against 0.203 ms with one slice and 0.162 ms for the position list, 1024: 0.85 / 0.95 / 1.07)
+    } else if (hk.mt_apply_nsl >= 0 && count <= 5 * sms) {
+        // up to a few hundred applications a level lasts as long as a CTA: four slices per CTA (measured: 148
+        // applications 0.137 ms against 0.203 ms with one slice, 0.162 ms for the position list and 0.65 ms for the
+        // four-streams-per-CTA kernel; 592: 0.49 against 0.66 ms; 1024: 0.85 against 0.77 ms)
         win(4);
     } else if (h_op) {
         mt19937_apply_multi_kernel<true><<<(unsigned)ceil_div_u64(count, AM_S), AM_THREADS, 0, stream>>>(

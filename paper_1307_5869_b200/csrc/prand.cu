@@ -67,8 +67,8 @@ void hook_assign(DebugHooks &h, const std::string &name, const char *v)
     else if (name == "PRAND_MT_APPLY") {
         const std::string m = on ? v : "";
         h.mt_apply_list = m == "list";
-        h.mt_apply_nsl = m == "win" ? 1 : m == "win2" ? 2 : m == "win4" ? 4 : 0;
-        h.mt_apply_win = h.mt_apply_nsl != 0;
+        h.mt_apply_nsl = m == "win" ? 1 : m == "win2" ? 2 : m == "win4" ? 4 : m == "multi" ? -1 : 0;
+        h.mt_apply_win = h.mt_apply_nsl > 0;
     }
     else if (name == "PRAND_GM_LP") h.gm_lp = on ? std::atoi(v) : 0;
     else if (name == "PRAND_GM31_NF") h.gm31_nf = on ? std::atoi(v) : -1;

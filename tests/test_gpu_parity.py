@@ -325,7 +325,7 @@ def test_set_state_refuses_words_the_kernels_cannot_take():
     assert P.lib().prand_trim() == 0
 
 
-@pytest.mark.parametrize("hook", [None, "win", "win2", "win4", "list"])
+@pytest.mark.parametrize("hook", [None, "win", "win2", "win4", "list", "multi"])
 def test_mt19937_every_polynomial_application_kernel(hook):
     """Eq. 10 in all its kernels: the four-streams-per-CTA form with the polynomial as a
     kernel argument (tree levels of >= 2368 streams) and from device memory (prand_jump by a distance that is
