@@ -1754,7 +1754,15 @@ cudaError_t mt19937_generate(cudaStream_t stream, const GenArgs &a, LaunchInfo *
     case 3:
         li->kernel = "mt19937_cgen<CS=4>";
         return a.dtype == DT_U32 ? launch_cgen<DT_U32>(stream, a) : launch_cgen<DT_F32>(stream, a);
-    case 6: li->kernel = "mt19937_wgen<CS=2>"; return dispatch_wdt<0>(stream, a);
+    case 6: {
+        // (a tensor map the driver refuses is not an error of the call: the cluster-pair kernel takes over)
+        li->kernel = "mt19937_wgen<CS=2>";
+        const cudaError_t e = dispatch_wdt<0>(stream, a);
+        if (e != cudaErrorInvalidValue || debug_hooks().mt_cfg >= 0) return e;
+        (void)cudaGetLastError();
+        li->kernel = "mt19937_gen<S=4,T=208,pair>";
+        return dispatch_dt<4, 208, 1, 6, true>(stream, a);
+    }
     case 4: li->kernel = "mt19937_tgen<S=4,T=208,pair>"; return dispatch_tdt<4, 208, 1, 6, true>(stream, a);
     case 5: li->kernel = "mt19937_tgen<S=8,T=104>"; return dispatch_tdt<8, 104, 2, 0, false>(stream, a);
     default: li->kernel = "mt19937_gen<S=4,T=208,pair>"; return dispatch_dt<4, 208, 1, 6, true>(stream, a);

@@ -190,8 +190,12 @@ def test_plan_covers_all_rows(gen):
                     assert cl % 4 == 0 and gen != "mt19937"
     # enough streams: never chunk
     assert P.prand_host_plan("lfsr113", 2**20, 2048, "u32", 148) == (2048, 1)
-    # config 1 (1024 streams x 4096) must be cut to fill the GPU
-    assert P.prand_host_plan("lfsr113", 1024, 4096, "u32", 148)[1] > 1
+    # config 1 (1024 streams x 4096) must be cut to fill the GPU: small L2-resident outputs run one stream per
+    # thread, so 1024 threads x 64 sub-sections of 64 rows (a second wave would cost a whole sub-section)
+    assert P.prand_host_plan("lfsr113", 1024, 4096, "u32", 148) == (64, 64)
+    # the same streams with long rows (output beyond 64 MiB): four streams per thread, sub-sections fill 148 x 1024 threads
+    cl, nc = P.prand_host_plan("lfsr113", 1024, 2**20, "u32", 148)
+    assert nc * (1024 // 4) <= 148 * 1024 < 2 * nc * (1024 // 4) and cl % 32 == 0
 
 
 def test_section_plan_covers_the_array_exactly_once():
