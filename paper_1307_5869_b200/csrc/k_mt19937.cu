@@ -1254,8 +1254,8 @@ mt19937_cgen_kernel(const uint32_t *st_in, uint32_t *st_out, uint32_t *__restric
 // Two CTAs (8 adjacent streams) form a cluster and trade halves: rows [0, 320) of every turn are written by CTA
 // 0, rows [320, 640) by CTA 1, each for all 8 streams = full 32-byte sectors.  A compute warp writes the steps
 // that belong to its own CTA with plain shared stores and the others straight into the partner's staging
-// columns with st.async, which counts the bytes on the partner's "full" mbarrier (no fence, no flag); buffers
-// come back through "empty" mbarriers, the partner's by a remote arrive.  Nothing on the compute warps' path
+// columns with st.async, which counts the bytes on the partner's "full" mbarrier (no fence, no flag); a buffer
+// comes back through one "empty" mbarrier on which the helpers of both CTAs arrive (the partner's remotely).  Nothing on the compute warps' path
 // waits for a TMA store or a proxy fence.  Rows outside whole turns of the ring (the first 16, the last < 640)
 // take a plain warp-level path on a shared-memory copy of the ring.
 constexpr int WG_S = 4;                                   // streams = compute warps = helper warps per CTA
@@ -1364,13 +1364,13 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
     constexpr int TILE = WG_BOX * WG_COLS;                // elements per helper tile
     constexpr int SBUF = WG_COLS * WG_CP;                 // words per staging buffer
     // tiles [helper][NTB][TILE] of E, staging [NSB][8 columns][CP], rings [stream][640],
-    // mbarriers sfull[NSB], sempty[NSB], pempty[NSB]
+    // mbarriers sfull[NSB], sempty[NSB]
     extern __shared__ __align__(128) uint32_t smem[];
     E *tiles = reinterpret_cast<E *>(smem);
     uint32_t *staging = smem + WG_HW * WG_NTB * TILE * W32;
     uint32_t *rings = staging + WG_NSB * SBUF;
     const uint32_t bars = smem_addr(rings + WG_S * WG_XS);
-    const uint32_t sfull = bars, sempty = bars + 8 * WG_NSB, pempty = bars + 16 * WG_NSB;
+    const uint32_t sfull = bars, sempty = bars + 8 * WG_NSB;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     uint32_t rank;
     asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
@@ -1380,8 +1380,7 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
     if (threadIdx.x == 0) {
         for (int b = 0; b < WG_NSB; b++) {
             mbar_init(sfull + 8 * b, WG_S);
-            mbar_init(sempty + 8 * b, WG_S);
-            mbar_init(pempty + 8 * b, WG_S);
+            mbar_init(sempty + 8 * b, 2 * WG_S);             // our four helper blocks and the partner's four
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -1396,7 +1395,7 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
         const int h = (warp - WG_S) % WG_S, par = (warp - WG_S) / WG_S;
         E *my = tiles + (warp - WG_S) * WG_NTB * TILE;
         const uint32_t my_s = smem_addr(my);
-        const uint32_t peer_pempty = map_to_cta(pempty, peer);
+        const uint32_t peer_sempty = map_to_cta(sempty, peer);
         const int x = (int)(sc0 * W32);
         const int y0 = 16 + WG_HALF * (int)rank + WG_BOX * h;
         const uint32_t *sp0 = staging + (lane & 1) * (WG_S * WG_CP) + h * WG_BOX + (lane >> 1);
@@ -1418,7 +1417,7 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
             __syncwarp();
             if (lane == 0) {
                 mbar_arrive(sempty + 8 * b);
-                mbar_arrive_cluster(peer_pempty + 8 * b);
+                mbar_arrive_cluster(peer_sempty + 8 * b);
                 tma_store_2d(&tmap, my_s + tb * (uint32_t)(TILE * sizeof(E)), x, y0 + WG_XS * (int)u);
             }
         }
@@ -1446,10 +1445,10 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
             const uint32_t rfull = map_to_cta(sfull, peer);
             for (uint32_t u = 0; u < turns; u++) {
                 const uint32_t b = u % WG_NSB, ph = ((u / WG_NSB) - 1u) & 1u;
-                // both staging columns of this turn must have been read out (here by our helpers, there by the partner's)
+                // both staging columns of this turn must have been read out, here by our helpers and there by the partner's:
+                // ONE barrier counts all eight (every mbarrier operation costs the compute warp ~100 clocks)
                 if (u >= WG_NSB) {
                     mbar_wait_sleep(sempty + 8 * b, ph);
-                    mbar_wait_sleep(pempty + 8 * b, ph);
                 }
                 if (rank == 0) wg_turn<0, HI>(r, lcol + b * SBUF, rcol + b * (uint32_t)(SBUF * 4), rfull + 8 * b, ge16, ge17, ge29, l17, l29, c);
                 else wg_turn<1, HI>(r, lcol + b * SBUF, rcol + b * (uint32_t)(SBUF * 4), rfull + 8 * b, ge16, ge17, ge29, l17, l29, c);
@@ -1482,7 +1481,7 @@ template <int DT, int HI> cudaError_t launch_wgen(cudaStream_t stream, const Gen
     typedef typename OutElem<DT>::type E;
     auto kern = mt19937_wgen_kernel<DT, HI>;
     const size_t smem = (size_t)WG_HW * WG_NTB * WG_BOX * WG_COLS * sizeof(E) + (size_t)WG_NSB * WG_COLS * WG_CP * 4 +
-                        (size_t)WG_S * WG_XS * 4 + 3 * WG_NSB * 8;
+                        (size_t)WG_S * WG_XS * 4 + 2 * WG_NSB * 8;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const uint32_t w32 = (uint32_t)(sizeof(E) / 4);
