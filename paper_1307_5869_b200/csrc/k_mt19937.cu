@@ -1266,7 +1266,7 @@ constexpr int WG_HALF = WG_XS / 2;                        // rows per CTA and tu
 constexpr int WG_HSTEPS = WG_RING / 2;                    // steps per CTA and turn
 constexpr int WG_BOX = WG_HALF / WG_S;                    // rows per helper and turn: one TMA box of 80 rows x 8 streams
 constexpr int WG_CP = WG_HALF + 4;                        // staging column pitch: the two CTAs' columns 16 banks apart
-constexpr int WG_NSB = 3;                                 // staging buffers
+constexpr int WG_NSB = 4;                                 // staging buffers (even: the compute warps wait for two at a time)
 constexpr int WG_HW = 2 * WG_S;                           // helper warps: two per row block, taking turns
 constexpr int WG_NTB = 2;                                 // tile buffers per helper
 constexpr int WG_THREADS = 32 * (WG_S + WG_HW);
@@ -1282,6 +1282,18 @@ __device__ __forceinline__ void mbar_wait_sleep(uint32_t a, uint32_t parity)
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(done) : "r"(a), "r"(parity) : "memory");
         if (done) break;
+        __nanosleep(40);
+    }
+}
+// two barriers at once: the polls are issued back to back, so their latencies overlap
+__device__ __forceinline__ void mbar_wait_sleep2(uint32_t a0, uint32_t p0, uint32_t a1, uint32_t p1)
+{
+    for (;;) {
+        uint32_t d0, d1;
+        asm volatile("{\n\t.reg .pred p, q;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%2], %3;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 q, [%4], %5;\n\tselp.u32 %0, 1, 0, p;\n\tselp.u32 %1, 1, 0, q;\n\t}"
+                     : "=r"(d0), "=r"(d1) : "r"(a0), "r"(p0), "r"(a1), "r"(p1) : "memory");
+        if (d0 & d1) break;
         __nanosleep(40);
     }
 }
@@ -1447,8 +1459,9 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
                 const uint32_t b = u % WG_NSB, ph = ((u / WG_NSB) - 1u) & 1u;
                 // both staging columns of this turn must have been read out, here by our helpers and there by the partner's:
                 // ONE barrier counts all eight (every mbarrier operation costs the compute warp ~100 clocks)
-                if (u >= WG_NSB) {
-                    mbar_wait_sleep(sempty + 8 * b, ph);
+                if (u >= WG_NSB && (u & 1u) == 0) {         // this turn's buffer and the next one's
+                    const uint32_t u1 = u + 1;
+                    mbar_wait_sleep2(sempty + 8 * b, ph, sempty + 8 * (u1 % WG_NSB), ((u1 / WG_NSB) - 1u) & 1u);
                 }
                 if (rank == 0) wg_turn<0, HI>(r, lcol + b * SBUF, rcol + b * (uint32_t)(SBUF * 4), rfull + 8 * b, ge16, ge17, ge29, l17, l29, c);
                 else wg_turn<1, HI>(r, lcol + b * SBUF, rcol + b * (uint32_t)(SBUF * 4), rfull + 8 * b, ge16, ge17, ge29, l17, l29, c);
