@@ -289,19 +289,19 @@ mrg32k3a_gen_fp64y_kernel(const uint32_t *st_in, uint32_t *st_out,
 // ---- sections of a single sequence, float64 (prand_generate_seq_f64; the paper's Table 7 task) -------
 // The array layout is PRAND's contiguous one, out[c * sec_len + i].  A warp owns 32 V
 // consecutive sections, lane k the sections k, k + 32, ...  It collects 16 rows of its sections in a
-// shared-memory tile (pitch 17 doubles: a lane's stores hit 16 different bank pairs, conflict-free) and
+// shared-memory tile (pitch 18 doubles: 16-byte aligned row pairs, 128-bit shared stores and loads conflict-free) and
 // writes them section by section: eight lanes store the 128 contiguous bytes of one section's 16 numbers,
 // so a warp store covers four full lines.  V = 1 with up to 2^17 sections fills the GPU with one wave of
 // 28 warps per SM; V = 2 serves fewer, longer sections.  The last section's state after its last row is
 // the state of the whole sequence after `length` numbers: it goes to st_last, no final jump is needed.
-constexpr int SEQ_ROWS = 16, SEQ_PITCH = 17;               // tile[section][row], pitch in doubles
+constexpr int SEQ_ROWS = 16, SEQ_PITCH = 18;               // tile[section][row], pitch in doubles (16-byte rows pairs)
 
 template <int V>
 __global__ void __launch_bounds__(GEN_THREADS, V == 1 ? 7 : 1)
 mrg32k3a_seq_f64_kernel(const uint32_t *st_in, uint32_t *st_last, double *__restrict__ out, uint64_t n_sections,
                         uint64_t sec_len, uint64_t length)
 {
-    __shared__ double tile_all[GEN_THREADS / 32][32 * V * SEQ_PITCH];
+    __shared__ __align__(16) double tile_all[GEN_THREADS / 32][32 * V * SEQ_PITCH];
     double *tile = tile_all[threadIdx.x >> 5];
     const int lane = threadIdx.x & 31;
     const uint64_t warp_sec0 = ((uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u)) * V;   // first section of the warp
@@ -320,6 +320,45 @@ mrg32k3a_seq_f64_kernel(const uint32_t *st_in, uint32_t *st_last, double *__rest
     const bool has_last = warp_sec0 + 32 * V > last;       // this warp owns the last section ...
     const int last_v = has_last ? (int)((last - warp_sec0) >> 5) : 0;   // ... as recurrence last_v of lane (last - warp_sec0) % 32
     const bool owns_last = has_last && lane == (int)((last - warp_sec0) & 31);
+    constexpr int LPS = SEQ_ROWS / 2;                      // lanes per section: each stores two doubles
+    const int sub = lane / LPS, piece = lane % LPS;
+    // Warps whose 32 V sections all exist and are all full-length (every warp but the array's last one) take the
+    // lean path: no row or section checks, one running pointer, tile offsets as immediates -- the checks, 64-bit
+    // address products and snapshot tests of the general path cost more instructions than the recurrence itself
+    // (ncu: 41 instructions per number against 27 in the bulk kernel; issue slots bound this kernel, not HBM).
+    if (!has_last && warp_sec0 + 32 * V <= n_sections) {
+        double *dst0 = out + (warp_sec0 + sub) * sec_len + 2 * piece;
+        const uint64_t kstride = (uint64_t)(32 / LPS) * sec_len;
+        const double *tsrc = tile + sub * SEQ_PITCH + 2 * piece;
+#pragma unroll 1
+        for (uint64_t i0 = 0; i0 < sec_len; i0 += SEQ_ROWS) {
+#pragma unroll
+            for (int r = 0; r < SEQ_ROWS; r += 2) {        // two rows per 128-bit shared store
+#pragma unroll
+                for (int v = 0; v < V; v++) {
+                    double o[2];
+#pragma unroll
+                    for (int h = 0; h < 2; h++) {
+                        const uint32_t nx = mrg_next_x(g[v].x1, g[v].x2, c1), ny = mrg_next_y(g[v].y0, g[v].y2);
+                        g[v].x2 = g[v].x1; g[v].x1 = g[v].x0; g[v].x0 = nx;
+                        g[v].y2 = g[v].y1; g[v].y1 = g[v].y0; g[v].y0 = ny;
+                        o[h] = mrg_output<DT_F64>(nx, ny);
+                    }
+                    *reinterpret_cast<double2 *>(tile + (32 * v + lane) * SEQ_PITCH + r) = make_double2(o[0], o[1]);
+                }
+            }
+            __syncwarp();
+            double *d = dst0 + i0;
+#pragma unroll
+            for (int k = 0; k < 32 * V / (32 / LPS); k++) {
+                const double2 t = *reinterpret_cast<const double2 *>(tsrc + k * (32 / LPS) * SEQ_PITCH);
+                store2(d, t.x, t.y);
+                d += kstride;
+            }
+            __syncwarp();
+        }
+        return;
+    }
 #pragma unroll 1
     for (uint64_t i0 = 0; i0 < sec_len; i0 += SEQ_ROWS) {
         const int snap = owns_last && last_rows >= i0 && last_rows < i0 + SEQ_ROWS ? (int)(last_rows - i0) : -1;
@@ -335,8 +374,6 @@ mrg32k3a_seq_f64_kernel(const uint32_t *st_in, uint32_t *st_last, double *__rest
             }
         }
         __syncwarp();
-        constexpr int LPS = SEQ_ROWS / 2;                  // lanes per section: each stores two doubles
-        const int sub = lane / LPS, piece = lane % LPS;
 #pragma unroll 4
         for (int k = 0; k < 32 * V / (32 / LPS); k++) {
             const int sl = (32 / LPS) * k + sub;           // section within the warp
