@@ -660,7 +660,9 @@ int ensure_chunk_ops(prand_state *st, uint64_t chunk_len, uint64_t n_chunks, cud
     return PRAND_OK;
 }
 
-int generate(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t stream)
+// peek: the numbers are produced but the streams do not advance (the advanced state goes to the spare buffer and is
+// dropped) -- what the skip-per-step generator needs before it jumps
+int generate(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t stream, bool peek = false)
 {
     if (!st || (!out && n)) return PRAND_ERR_ARG;
     if (n == 0) return PRAND_OK;
@@ -681,13 +683,15 @@ int generate(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t str
     a.clean = st->gm_clean;
     a.st_in = st->d_state[st->cur];
     a.st_out = st->d_state[st->cur];
-    if (a.n_chunks > 1) {
+    if (a.n_chunks > 1 || peek) {
         // chunk c reads the start state while the last chunk writes the final one: separate buffers
         int rc = ensure_second_buffer(st);
         if (rc) return rc;
-        rc = ensure_chunk_ops(st, a.chunk_len, a.n_chunks, stream);
-        if (rc) return rc;
-        a.chunk_ops = st->d_chunk_ops;
+        if (a.n_chunks > 1) {
+            rc = ensure_chunk_ops(st, a.chunk_len, a.n_chunks, stream);
+            if (rc) return rc;
+            a.chunk_ops = st->d_chunk_ops;
+        }
         a.st_out = st->d_state[1 - st->cur];
     }
     LaunchInfo li = {"", 0};
@@ -698,6 +702,7 @@ int generate(prand_state *st, void *out, uint64_t n, int dtype, cudaStream_t str
     else e = gm_generate(stream, st->gen, a, &li);
     if (e != cudaSuccess) return cuda_fail(e);
     note(st, li);
+    if (peek) return PRAND_OK;
     if (a.n_chunks > 1) st->cur = 1 - st->cur;
     if (n >= 16) st->gm_clean = true;
     return PRAND_OK;
@@ -876,7 +881,7 @@ int generate_seq(prand_state *st, void *out, uint64_t length, int dtype, cudaStr
 // prand_generate_strided_* (SURVEY.md 8(f)4): the sequence that skips ahead after every output
 // (Table 3 PAPER.md:249-275 tests such sequences for skips of 2^n).  Row i holds every
 // stream's output at position P + i * stride: the output is produced from a copy of the state, the
-// state itself jumps by `stride` with one prepared operator.
+// state itself jumps by `stride` with one prepared operator: two launches per row, no copy of the state.
 namespace {
 int generate_strided(prand_state *st, void *out, uint64_t n, int dtype, Dist stride, cudaStream_t stream)
 {
@@ -893,11 +898,8 @@ int generate_strided(prand_state *st, void *out, uint64_t n, int dtype, Dist str
     if (rc) return rc;
     const bool clean0 = st->gm_clean;
     for (uint64_t i = 0; i < n; i++) {
-        const int cur = st->cur;
-        CU(cudaMemcpyAsync(st->d_state[1 - cur], st->d_state[cur], st->bytes, cudaMemcpyDeviceToDevice, stream));
-        st->cur = 1 - cur;                                   // one output from the copy
-        rc = generate(st, (char *)out + i * st->ns * esz, 1, dtype, stream);
-        st->cur = cur;
+        // one output per stream without advancing it (the stepped state lands in the spare buffer: no state copy)
+        rc = generate(st, (char *)out + i * st->ns * esz, 1, dtype, stream, true);
         if (rc) return rc;
         rc = jump_launch(st, stream);
         if (rc) return rc;
