@@ -363,6 +363,28 @@ def jump_methods(torch, P):
     return out
 
 
+def device_api_rates(torch, P):
+    """the device-callable API (include/prand_device.cuh) through the library's example kernels --
+    one thread per stream calling next_u32() -- beside the bulk kernel on the same family (65,536 streams x 2048 u32;
+    MT19937: one warp per stream, 2048 streams x 65,536), and stream initialisation by skip-ahead on the device
+    (prand_device_api_init_fill: skipahead + 16 numbers per stream).  CUDA-event medians of 5 calls after 2 warm-ups."""
+    out = {}
+    for gen, seed, ns, L, n in (("lfsr113", 12345, 65536, 2**33, 2048), ("mrg32k3a", 12345, 65536, 2**76, 2048),
+                                ("gm31", 1, 65536, 2**26, 2048), ("gq58.4", 1, 65536, 2**26, 2048),
+                                ("mt19937", 5489, 2048, 2**64, 65536)):
+        g = P.Generator(gen, seed, ns, L)
+        bulk = statistics.median(event_ms(torch, lambda: g.generate(n, "u32"), 5, warm=2))
+        dev = statistics.median(event_ms(torch, lambda: g.device_api_fill(n, "u32"), 5, warm=2))
+        g.close()
+        b = P.Generator(gen, seed, 1, 0)
+        ini = statistics.median(event_ms(torch, lambda: b.device_api_init_fill(ns if gen != "mt19937" else 256, L, 16, "u32"), 5, warm=2))
+        b.close()
+        out[gen] = {"n_streams": ns, "n_per_stream": n, "bulk_gnumbers_per_s": ns * n / bulk / 1e6,
+                    "device_api_gnumbers_per_s": ns * n / dev / 1e6,
+                    "device_init_streams": ns if gen != "mt19937" else 256, "device_init_ms": ini}
+    return out
+
+
 def run_ours(args, w):
     import torch
     import paper_1307_5869_b200 as P
@@ -500,6 +522,7 @@ def run_ours(args, w):
             print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
         line["per_config"] = rows
         line["jump_methods"] = jump_methods(torch, P)
+        line["device_api"] = device_api_rates(torch, P)
         line["per_config_note"] = ("generation call alone (prand_generate_* / prand_generate_seq_*), CUDA-event median of "
                                    f"{args.config_steps} calls after 3 warm-ups, 256 MB written before each call (L2 flush); "
                                    "frac: hbm = algorithmic bytes (output + 2 x state) / gen_ms / MEASURED_PEAKS hbm_gbs; "
