@@ -64,6 +64,10 @@ cudaError_t lfsr113_jump(cudaStream_t, const JumpArgs &, LaunchInfo *);
 // one warp per stream; a.ops is not used
 cudaError_t lfsr113_table_jump(cudaStream_t, const JumpArgs &, uint64_t mant, unsigned log2, LaunchInfo *);
 cudaError_t lfsr113_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
+// sections of one sequence in PRAND's contiguous layout out[c * sec_len + i] (sec_len a multiple of 32, out 16-byte
+// aligned); st_in = the section family's state (structure of arrays); the caller advances the sequence's own state
+cudaError_t lfsr113_seq(cudaStream_t, const void *st_in, void *out, int dtype, uint64_t n_sections, uint64_t sec_len,
+                        uint64_t length, LaunchInfo *);
 // small outputs (they stay in L2) from few streams: one stream per thread, so that four times as many threads share
 // the work and a sub-section's jump is paid once per 64 rows of one stream instead of four (C1: 18 -> 14 us)
 inline bool lfsr113_narrow(uint64_t ns, uint64_t n, int dtype, int sms)

@@ -272,6 +272,75 @@ lfsr113_gen_kernel(const uint32_t *st_in, uint32_t *st_out,
     }
 }
 
+// ---- sections of a single sequence (prand_generate_seq_*; Table 5) ----------------------
+// The array layout is PRAND's contiguous one, out[c * sec_len + i].  One thread per section (lane = section); a
+// warp collects a block of 32 rows of its 32 sections in a shared-memory tile (pitch 33: conflict-free both ways)
+// and writes it section by section: 16 bytes per lane, the lanes of a section storing its 32 consecutive numbers
+// as one contiguous run (128 bytes for u32 / f32, 256 for f64).  No scratch array, no transposition pass.
+template <int DT, int N>
+__device__ __forceinline__ void lfsr113_emit_tile(LfsrBits<1> &b, typename OutElem<DT>::type *t)
+{
+    if constexpr (N <= 32) {
+        t[N - 1] = convert<DT>(b.c1[0].template output<N>() ^ b.c2[0].template output<N>() ^
+                               b.c3[0].template output<N>() ^ b.c4[0].template output<N>());
+        lfsr113_emit_tile<DT, N + 1>(b, t);
+    }
+}
+
+template <int DT>
+__global__ void __launch_bounds__(GEN_THREADS)
+lfsr113_seq_kernel(const uint32_t *st_in, typename OutElem<DT>::type *__restrict__ out, uint64_t n_sections,
+                   uint64_t sec_len, uint64_t length)
+{
+    typedef typename OutElem<DT>::type T;
+    constexpr int PITCH = 33;
+    constexpr int EPL = 16 / (int)sizeof(T);               // elements per lane and store (4 or 2)
+    constexpr int LPS = 32 / EPL;                          // lanes per section
+    constexpr int SPP = 32 / LPS;                          // sections per pass
+    __shared__ T tile_all[GEN_THREADS / 32][32 * PITCH];
+    T *tile = tile_all[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const uint64_t warp_sec0 = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u);
+    if (warp_sec0 >= n_sections) return;                   // whole warp
+    const uint64_t sec = warp_sec0 + lane < n_sections ? warp_sec0 + lane : n_sections - 1;
+    LfsrBits<1> b;
+    b.c1[0].load(st_in[0 * n_sections + sec]);
+    b.c2[0].load(st_in[1 * n_sections + sec]);
+    b.c3[0].load(st_in[2 * n_sections + sec]);
+    b.c4[0].load(st_in[3 * n_sections + sec]);
+    const uint64_t last = n_sections - 1, last_rows = length - last * sec_len;
+    const bool whole = warp_sec0 + 32 <= n_sections && (warp_sec0 + 32 <= last || last_rows == sec_len);
+    const int sub = lane / LPS, piece = lane % LPS;
+    T *dst0 = out + (warp_sec0 + sub) * sec_len + EPL * piece;
+    const T *tsrc = tile + sub * PITCH + EPL * piece;
+#pragma unroll 1
+    for (uint64_t i0 = 0; i0 < sec_len; i0 += 32) {        // (sec_len is a multiple of 32)
+        lfsr113_emit_tile<DT, 1>(b, tile + lane * PITCH);
+        b.c1[0].next_block(); b.c2[0].next_block(); b.c3[0].next_block(); b.c4[0].next_block();
+        __syncwarp();
+        T *d = dst0 + i0;
+#pragma unroll
+        for (int k = 0; k < 32 / SPP; k++) {
+            T v[EPL];
+#pragma unroll
+            for (int e = 0; e < EPL; e++) v[e] = tsrc[k * SPP * PITCH + e];
+            if (whole) {
+                store_vec<EPL>(d, v);
+            } else {
+                const uint64_t c = warp_sec0 + SPP * k + sub;
+                if (c < n_sections) {
+                    const uint64_t rows = c == last ? last_rows : sec_len, row = i0 + EPL * piece;
+#pragma unroll
+                    for (int e = 0; e < EPL; e++)
+                        if (row + e < rows) store1(d + e, v[e]);
+                }
+            }
+            d += (uint64_t)SPP * sec_len;
+        }
+        __syncwarp();
+    }
+}
+
 template <int V, int DT>
 cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
 {
@@ -303,6 +372,20 @@ cudaError_t lfsr113_jump(cudaStream_t stream, const JumpArgs &a, LaunchInfo *li)
                                                     (uint32_t *)a.st_out, a.n_streams,
                                                     (const LfsrOp *)a.ops, a.idx0, a.idx_stride);
     li->kernel = "lfsr113_jump";
+    li->launches = 1;
+    return cudaGetLastError();
+}
+
+cudaError_t lfsr113_seq(cudaStream_t stream, const void *st_in, void *out, int dtype, uint64_t n_sections, uint64_t sec_len,
+                        uint64_t length, LaunchInfo *li)
+{
+    const unsigned blocks = (unsigned)ceil_div_u64(ceil_div_u64(n_sections, 32) * 32, GEN_THREADS);
+    switch (dtype) {
+    case DT_U32: lfsr113_seq_kernel<DT_U32><<<blocks, GEN_THREADS, 0, stream>>>((const uint32_t *)st_in, (uint32_t *)out, n_sections, sec_len, length); break;
+    case DT_F32: lfsr113_seq_kernel<DT_F32><<<blocks, GEN_THREADS, 0, stream>>>((const uint32_t *)st_in, (float *)out, n_sections, sec_len, length); break;
+    default: lfsr113_seq_kernel<DT_F64><<<blocks, GEN_THREADS, 0, stream>>>((const uint32_t *)st_in, (double *)out, n_sections, sec_len, length); break;
+    }
+    li->kernel = "lfsr113_seq";
     li->launches = 1;
     return cudaGetLastError();
 }

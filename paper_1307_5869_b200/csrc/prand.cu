@@ -861,6 +861,13 @@ int generate_seq(prand_state *st, void *out, uint64_t length, int dtype, cudaStr
         note(st, li);
         return PRAND_OK;
     }
+    if (st->gen == PRAND_LFSR113 && (uintptr_t)out % 16 == 0) {
+        // one section per thread, 32-row blocks transposed through a per-warp shared-memory tile
+        LaunchInfo li;
+        CU(lfsr113_seq(stream, c->d_state[c->cur], out, dtype, S, L, length, &li));
+        note(st, li);
+        return prand_jump(st, length, 0, stream);          // the sequence has advanced by `length`
+    }
     void *tmp = nullptr;
     CU(dev_alloc(&tmp, (size_t)L * S * esz, stream));
     rc = generate(c, tmp, L, dtype, stream);
