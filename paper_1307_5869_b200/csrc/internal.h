@@ -81,6 +81,9 @@ cudaError_t mrg32k3a_generate(cudaStream_t, const GenArgs &, LaunchInfo *);
 // st_last (one stream) receives the state of the sequence after `length` numbers
 cudaError_t mrg32k3a_seq_f64(cudaStream_t, const void *st_in, void *st_last, double *out, uint64_t n_sections,
                              uint64_t sec_len, uint64_t length, LaunchInfo *);
+// the same layout for u32 / f32 outputs (sec_len a multiple of 32); the caller advances the sequence's own state
+cudaError_t mrg32k3a_seq4(cudaStream_t, const void *st_in, void *out, int dtype, uint64_t n_sections, uint64_t sec_len,
+                          uint64_t length, LaunchInfo *);
 cudaError_t gm_jump(cudaStream_t, int gen, const JumpArgs &, LaunchInfo *);
 cudaError_t gm_generate(cudaStream_t, int gen, const GenArgs &, LaunchInfo *);
 // streams [s_begin, s_end) = kn * stream(s - back) - qn * stream(s - 2 back) (eq. 2), in place

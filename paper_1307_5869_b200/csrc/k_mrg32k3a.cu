@@ -392,6 +392,65 @@ mrg32k3a_seq_f64_kernel(const uint32_t *st_in, uint32_t *st_last, double *__rest
     if (owns_last && last_rows == sec_len) mrg_store(st_last, 1, 0, g[last_v]);
 }
 
+// The same for four-byte outputs (u32, f32): one section per thread, blocks of 32 rows in a per-warp tile
+// [section][row] (pitch 33 words: conflict-free both ways), written section by section, eight lanes storing the 128
+// contiguous bytes of one section's 32 numbers.  Both components on the integer pipes (the FP64-pipe form of the
+// bulk kernel pays off only at the HBM rate, which this layout does not reach).  The caller advances the state of
+// the sequence itself (prand_jump by `length`).
+template <int DT>
+__global__ void __launch_bounds__(GEN_THREADS)
+mrg32k3a_seq4_kernel(const uint32_t *st_in, typename OutElem<DT>::type *__restrict__ out, uint64_t n_sections,
+                     uint64_t sec_len, uint64_t length)
+{
+    typedef typename OutElem<DT>::type T;
+    static_assert(sizeof(T) == 4, "four-byte outputs");
+    constexpr int PITCH = 33, LPS = 8, SPP = 4;            // lanes per section (4 numbers each), sections per pass
+    __shared__ T tile_all[GEN_THREADS / 32][32 * PITCH];
+    T *tile = tile_all[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const uint64_t warp_sec0 = (uint64_t)blockIdx.x * blockDim.x + (threadIdx.x & ~31u);
+    if (warp_sec0 >= n_sections) return;                   // whole warp
+    Mrg g = mrg_load(st_in, n_sections, warp_sec0 + lane < n_sections ? warp_sec0 + lane : n_sections - 1);
+    uint32_t c1 = C1;
+    asm volatile("" : "+r"(c1));
+    const uint64_t last = n_sections - 1, last_rows = length - last * sec_len;
+    const bool whole = warp_sec0 + 32 <= n_sections && (warp_sec0 + 32 <= last || last_rows == sec_len);
+    const int sub = lane / LPS, piece = lane % LPS;
+    T *dst0 = out + (warp_sec0 + sub) * sec_len + 4 * piece;
+    const T *tsrc = tile + sub * PITCH + 4 * piece;
+#pragma unroll 1
+    for (uint64_t i0 = 0; i0 < sec_len; i0 += 32) {        // (sec_len is a multiple of 32)
+#pragma unroll
+        for (int r = 0; r < 32; r++) {
+            const uint32_t nx = mrg_next_x(g.x1, g.x2, c1), ny = mrg_next_y(g.y0, g.y2);
+            g.x2 = g.x1; g.x1 = g.x0; g.x0 = nx;
+            g.y2 = g.y1; g.y1 = g.y0; g.y0 = ny;
+            tile[lane * PITCH + r] = mrg_output<DT>(nx, ny);
+        }
+        __syncwarp();
+        T *d = dst0 + i0;
+#pragma unroll
+        for (int k = 0; k < 32 / SPP; k++) {
+            T v[4];
+#pragma unroll
+            for (int e = 0; e < 4; e++) v[e] = tsrc[k * SPP * PITCH + e];
+            if (whole) {
+                store_vec<4>(d, v);
+            } else {
+                const uint64_t c = warp_sec0 + SPP * k + sub;
+                if (c < n_sections) {
+                    const uint64_t rows = c == last ? last_rows : sec_len, row = i0 + 4 * piece;
+#pragma unroll
+                    for (int e = 0; e < 4; e++)
+                        if (row + e < rows) store1(d + e, v[e]);
+                }
+            }
+            d += (uint64_t)SPP * sec_len;
+        }
+        __syncwarp();
+    }
+}
+
 template <int V, int DT> cudaError_t launch_gen(cudaStream_t stream, const GenArgs &a)
 {
     typedef typename OutElem<DT>::type T;
@@ -446,6 +505,19 @@ cudaError_t mrg32k3a_seq_f64(cudaStream_t stream, const void *st_in, void *st_la
             (const uint32_t *)st_in, (uint32_t *)st_last, out, n_sections, sec_len, length);
     }
     li->kernel = "mrg32k3a_seq_f64";
+    li->launches = 1;
+    return cudaGetLastError();
+}
+
+cudaError_t mrg32k3a_seq4(cudaStream_t stream, const void *st_in, void *out, int dtype, uint64_t n_sections, uint64_t sec_len,
+                          uint64_t length, LaunchInfo *li)
+{
+    const unsigned blocks = (unsigned)ceil_div_u64(ceil_div_u64(n_sections, 32) * 32, GEN_THREADS);
+    if (dtype == DT_U32)
+        mrg32k3a_seq4_kernel<DT_U32><<<blocks, GEN_THREADS, 0, stream>>>((const uint32_t *)st_in, (uint32_t *)out, n_sections, sec_len, length);
+    else
+        mrg32k3a_seq4_kernel<DT_F32><<<blocks, GEN_THREADS, 0, stream>>>((const uint32_t *)st_in, (float *)out, n_sections, sec_len, length);
+    li->kernel = "mrg32k3a_seq4";
     li->launches = 1;
     return cudaGetLastError();
 }

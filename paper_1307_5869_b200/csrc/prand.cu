@@ -861,6 +861,12 @@ int generate_seq(prand_state *st, void *out, uint64_t length, int dtype, cudaStr
         note(st, li);
         return PRAND_OK;
     }
+    if (st->gen == PRAND_MRG32K3A && dtype != DT_F64 && (uintptr_t)out % 16 == 0) {
+        LaunchInfo li;
+        CU(mrg32k3a_seq4(stream, c->d_state[c->cur], out, dtype, S, L, length, &li));
+        note(st, li);
+        return prand_jump(st, length, 0, stream);          // the sequence has advanced by `length`
+    }
     if (st->gen == PRAND_LFSR113 && (uintptr_t)out % 16 == 0) {
         // one section per thread, 32-row blocks transposed through a per-warp shared-memory tile
         LaunchInfo li;

@@ -247,7 +247,9 @@ def test_single_sequence_fill_equals_the_serial_generator(gen):
     need_gpu()
     seed = workloads.SEED.get(gen, 1)
     lengths = [100000, 7, 40001] if gen != "mt19937" else [30000, 5, 12345]
-    for dtype in (["u32", "f64"] if gen in ("mrg32k3a", "gm31") else ["u32"]):
+    # (LFSR113, MRG32K3A and MT19937 write the contiguous layout in place, with one kernel per element size)
+    for dtype in (["u32", "f32", "f64"] if gen in ("mrg32k3a", "lfsr113", "mt19937") else
+                  ["u32", "f64"] if gen == "gm31" else ["u32"]):
         g = P.Generator(gen, seed, 1, 0)
         g.jump(3)
         got = [g.generate_seq(n, dtype).cpu().numpy().view(NPDT[dtype]) for n in lengths]
