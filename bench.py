@@ -55,14 +55,16 @@ ALU_BOUND = {"gm19", "gm29", "gm31", "gm55", "gm61", "gq58.1", "gq58.3", "gq58.4
 def load_alu_counts():
     """Thread-instructions per number of the integer-bound generation kernels, as counted by ncu
     (smsp__inst_executed.sum x 32 / numbers) in the committed --set full captures: profiles/alu_counts.csv
-    is written from those captures (its `source` column names the details file), never edited by hand."""
+    is written from those captures (its `source` column names the details file), never edited by hand; the pipe
+    utilisations ncu measured in the same capture (ALU pipe, FMA-pipe cycles, issue slots) ride along."""
     import csv
     path = os.path.join(ROOT, "profiles", "alu_counts.csv")
     out = {}
     if os.path.exists(path):
         with open(path, newline="") as f:
             for row in csv.DictReader(f):
-                out[row["kernel"]] = (float(row["thread_instr_per_number"]), row["source"])
+                pipes = {k: float(row[k]) for k in ("alu_pipe_pct", "fma_pipe_cycles_pct", "issue_active_pct") if row.get(k)}
+                out[row["kernel"]] = (float(row["thread_instr_per_number"]), row["source"], pipes)
     return out
 
 
@@ -227,12 +229,12 @@ def roofline_of(w, kernel, k_ms, peak, peak_src, share=None, fill_gbs=None):
     traffic = load_traffic(kernel)
     if w.gen in ALU_BOUND:                         # integer-bound: report against the issue peak
         counts = load_alu_counts()
-        ipn, src = counts.get(kernel, (None, None))
+        ipn, src, pipes = counts.get(kernel, (None, None, {}))
         p_g = alu_peak_ginstr()
         a_g = ipn * w.numbers / (k_ms * 1e-3) / 1e9 if ipn else None
         r = {"bound": "alu", "achieved": a_g, "peak": p_g, "unit": "Gthread-instr/s",
              "frac": a_g / p_g if a_g else None, "traffic": traffic, "kernel": kernel, "kernel_ms": k_ms,
-             "thread_instr_per_number": ipn, "thread_instr_source": src,
+             "thread_instr_per_number": ipn, "thread_instr_source": src, "ncu_pipe_pct": pipes,
              "peak_source": "148 SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md 6.5, profiles/pipe_rates.md)",
              "out_gbs": out_gbs, "hbm_peak_gbs": peak, "frac_of_hbm": alg_gbs / peak}
     else:
@@ -318,7 +320,7 @@ def time_config(torch, P, w, steps, warmup, flush, peak, peak_src, device_index=
             "gen_ms": med, "gen_ms_best": min(gen_ms), "gnumbers_per_s": w.numbers / (med * 1e-3) / 1e9,
             "bound": roof["bound"], "frac": roof["frac"], "out_gbs": roof["out_gbs"],
             "algorithmic_bytes": algorithmic_bytes(w), "frac_of_hbm": roof.get("frac_of_hbm", roof["frac"]),
-            "thread_instr_per_number": roof.get("thread_instr_per_number"),
+            "thread_instr_per_number": roof.get("thread_instr_per_number"), "ncu_pipe_pct": roof.get("ncu_pipe_pct"),
             "init_ms": min(init_ms), "init_streams_per_s": w.n_streams / (min(init_ms) * 1e-3),
             "clocks": clk.summary()}
 
