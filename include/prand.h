@@ -131,8 +131,9 @@ int prand_generate_f64_host(prand_state *st, double *host_out, uint64_t n_per_st
  *   from its current position, i.e. exactly what `length` successive single-stream generate calls
  *   would have produced; afterwards the stream has advanced by `length`.  `out` is caller-owned DEVICE
  *   memory with `length` elements.  Unlike PRAND no divisibility of `length` by the
- *   number of sections is required (MT19937: no power of two).  The library allocates
- *   (stream-ordered) a scratch buffer of about `length` elements for the duration of the call.
+ *   number of sections is required (MT19937: no power of two).  LFSR113, MRG32K3A and MT19937 write `out`
+ *   in place when it is 16-byte aligned; the GM/GQ generators (and unaligned `out`) go through a stream-ordered
+ *   scratch buffer of about `length` elements that the library allocates for the duration of the call.
  */
 int prand_generate_seq_u32(prand_state *st, uint32_t *out, uint64_t length, void *cuda_stream);
 int prand_generate_seq_f32(prand_state *st, float *out, uint64_t length, void *cuda_stream);
@@ -144,7 +145,8 @@ int prand_generate_seq_f64(prand_state *st, double *out, uint64_t length, void *
  *   + s] = the output of stream s at position P_s + i * stride (P_s = its current position), stride =
  *   stride_mant * 2^stride_log2 >= 1; afterwards every stream has advanced n_per_stream * stride.
  *   One jump per output row (the operator is prepared once): meant for testing skip-ahead sequences,
- *   not for bulk throughput.  The library keeps a second copy of the state while it runs.
+ *   not for bulk throughput.  The library keeps a second state buffer while it runs (the stepped state of the
+ *   output row lands there; the state itself is not copied).
  */
 int prand_generate_strided_u32(prand_state *st, uint32_t *out, uint64_t n_per_stream, uint64_t stride_mant,
                                unsigned stride_log2, void *cuda_stream);
