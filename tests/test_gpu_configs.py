@@ -105,7 +105,14 @@ def test_c5_sweep_full_size_sampled(w):
     check_config(w, 6 if w.gen == "mt19937" else 40)
 
 
-@pytest.mark.parametrize("w", workloads.T7, ids=lambda w: w.name)
+# in-place sequence fills beside the paper's two: a ragged length that leaves the last section short (and the last
+# warp of sections partly empty), with enough sections (> 32,768) to reach the kernels the Table 7 fills use
+SEQ_RAGGED = [workloads.Workload("seq-mrg32k3a-f64", "mrg32k3a", 12345, 1, 0, 2 ** 27 + 12345, "f64", True),
+              workloads.Workload("seq-mrg32k3a-u32", "mrg32k3a", 12345, 1, 0, 2 ** 27 + 12345, "u32", True),
+              workloads.Workload("seq-lfsr113-f32", "lfsr113", 12345, 1, 0, 2 ** 27 + 12345, "f32", True)]
+
+
+@pytest.mark.parametrize("w", workloads.T7 + SEQ_RAGGED, ids=lambda w: w.name)
 def test_t7_sequence_fill_full_size_sampled_sections(w):
     """The paper's Table 7 task at its size (one sequence, 2^29 doubles in device memory)
     through prand_generate_seq_f64, in the section plan the bench times: ALL numbers of >= 16 sampled
@@ -132,8 +139,9 @@ def test_t7_sequence_fill_full_size_sampled_sections(w):
     base = oracle.State(w.gen, w.seed).jump(5)
     for c in sorted(picks):
         lo, hi = c * L, min(n, (c + 1) * L)
-        got = out[lo:hi].cpu().numpy().view(np.uint64)
-        want = base.copy().jump(lo).fill(hi - lo, w.dtype).view(np.uint64)
+        bits = np.uint64 if w.dtype == "f64" else np.uint32
+        got = out[lo:hi].cpu().numpy().view(bits)
+        want = base.copy().jump(lo).fill(hi - lo, w.dtype).view(bits)
         if not np.array_equal(got, want):
             i = int(np.argmax(got != want))
             raise AssertionError(f"{w.name} [{kernel}] section {c}: {(got != want).sum()} of {len(got)} differ, first at {i}")
