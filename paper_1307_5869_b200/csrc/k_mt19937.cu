@@ -1266,7 +1266,7 @@ constexpr int WG_HALF = WG_XS / 2;                        // rows per CTA and tu
 constexpr int WG_HSTEPS = WG_RING / 2;                    // steps per CTA and turn
 constexpr int WG_BOX = WG_HALF / WG_S;                    // rows per helper and turn: one TMA box of 80 rows x 8 streams
 constexpr int WG_CP = WG_HALF + 4;                        // staging column pitch: the two CTAs' columns 16 banks apart
-constexpr int WG_NSB = 4;                                 // staging buffers (even: the compute warps wait for two at a time)
+constexpr int WG_NSB = 6;                                 // staging buffers (even: the compute warps wait for two at a time)
 constexpr int WG_HW = 2 * WG_S;                           // helper warps: two per row block, taking turns
 constexpr int WG_NTB = 2;                                 // tile buffers per helper
 constexpr int WG_THREADS = 32 * (WG_S + WG_HW);
