@@ -63,7 +63,8 @@ enum prand_error {
     PRAND_ERR_CUDA = -5,       /* a CUDA runtime call failed; prand_last_cuda_error() has it  */
     PRAND_ERR_SIZE = -6,       /* byte count does not match prand_state_bytes()               */
     PRAND_ERR_ALLOC = -7,      /* host or device allocation failed                            */
-    PRAND_ERR_INTERNAL = -8    /* MT19937: the characteristic polynomial failed its self-check  */
+    PRAND_ERR_INTERNAL = -8,   /* MT19937: the characteristic polynomial failed its self-check  */
+    PRAND_ERR_CAPACITY = -9    /* request larger than the fixed capacity of a no-allocation entry point */
 };
 
 /*
@@ -138,6 +139,44 @@ int prand_generate_f64_host(prand_state *st, double *host_out, uint64_t n_per_st
 int prand_generate_seq_u32(prand_state *st, uint32_t *out, uint64_t length, void *cuda_stream);
 int prand_generate_seq_f32(prand_state *st, float *out, uint64_t length, void *cuda_stream);
 int prand_generate_seq_f64(prand_state *st, double *out, uint64_t length, void *cuda_stream);
+
+/*
+ * prand_lfsr113_seq_noalloc_u32 -- the single-sequence fill (Table 5) for callers
+ *   that must not allocate device memory.
+ *
+ *   Why it exists: all other generating calls work on a prand_state, which prand_init creates from the library's
+ *   memory pool, and prand_generate_seq_* allocates its table of section start states on demand.  Code that runs
+ *   where the CUDA allocator is off limits -- inside a latency-critical loop that owns one arena reserved at
+ *   start-up, under a framework whose caching allocator owns the device and tolerates no foreign cudaMalloc or
+ *   pool growth, in a plug-in that may only use the buffers its host application hands it, or so close to the
+ *   memory limit that an allocation could fail or stall the device -- cannot use those calls at that point.  This
+ *   one calls no cudaMalloc / cudaFree / pool routine and no library routine that allocates device memory: the
+ *   section table and the jump operators live in a fixed 520 KiB __device__ array inside libprand.so (each GPU
+ *   that loads the library holds its copy until the process exits).
+ *
+ *   d_state  DEVICE pointer to 4 x u32, caller-owned: the LFSR113 state in the canonical layout of prand_get_state
+ *            for one stream (z1..z4).  Read as the start of the sequence and overwritten with the state after
+ *            `length` numbers, so successive calls continue the sequence and the words can be given to
+ *            prand_set_state.  The words are not validated here (a component whose significant top bits are all
+ *            zero stays zero, as prand_init / prand_set_state would have refused).
+ *   out      DEVICE pointer, `length` u32, 16-byte aligned, caller-owned.  out[j] = output number j of the
+ *            sequence counted from the state's position: exactly what prand_generate_seq_u32 writes.
+ *   length   at most PRAND_NOALLOC_MAX_LENGTH numbers per call (the array holds PRAND_NOALLOC_MAX_SECTIONS
+ *            section start states and a section is kept to at most 65,536 numbers); more returns
+ *            PRAND_ERR_CAPACITY and nothing is launched -- fill a longer array with several calls.  0 is a no-op.
+ *   Errors   PRAND_ERR_ARG (null or misaligned pointer), PRAND_ERR_CAPACITY, PRAND_ERR_CUDA.
+ *
+ *   The work (two operator uploads of at most 8 KiB from host memory, three kernel launches) is asynchronous on
+ *   `cuda_stream`.  The FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, with
+ *   that device current), which may load the library's module there: make that first call before any stream
+ *   capture begins.  All calls on a device share the one array, which keeps what the previous call wrote; nothing
+ *   in it needs clearing (each call writes every word it reads), but two calls whose GPU work overlaps -- streams
+ *   without an ordering between them, or concurrent host threads -- race on it and give wrong numbers.  Keep the
+ *   calls on one stream or order them with events.
+ */
+#define PRAND_NOALLOC_MAX_SECTIONS 32768u
+#define PRAND_NOALLOC_MAX_LENGTH (1ull << 31)
+int prand_lfsr113_seq_noalloc_u32(uint32_t *d_state, uint32_t *out, uint64_t length, void *cuda_stream);
 
 /*
  * prand_generate_strided_{u32,f32,f64} -- the generator that skips ahead after every output

@@ -40,6 +40,7 @@ _SIGS = {
     "prand_generate_seq_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_generate_seq_f32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_generate_seq_f64": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
+    "prand_lfsr113_seq_noalloc_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
     "prand_state_device_ptr": (C.c_void_p, [C.c_void_p]),
     "prand_state_n_streams": (C.c_uint64, [C.c_void_p]),
     "prand_device_api_fill_u32": (C.c_int, [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]),
@@ -196,6 +197,17 @@ def prand_get_state(state: int) -> bytes:
 
 def prand_set_state(state: int, canon: bytes) -> None:
     _check(lib().prand_set_state(state, canon, len(canon)), "prand_set_state")
+
+
+def prand_lfsr113_seq_noalloc_u32(d_state_ptr: int, out_ptr: int, length: int, stream=None) -> None:
+    """Single-sequence LFSR113 fill that allocates no device memory (include/prand.h): for callers that may not touch
+    the CUDA allocator where they need the numbers.  ``d_state_ptr``: 4 u32 of the caller's device memory (canonical
+    state, advanced in place); ``out_ptr``: ``length`` u32, 16-byte aligned; ``length`` <= NOALLOC_MAX_LENGTH."""
+    _check(lib().prand_lfsr113_seq_noalloc_u32(d_state_ptr, out_ptr, length, _stream_ptr(stream)),
+           "prand_lfsr113_seq_noalloc_u32")
+
+
+NOALLOC_MAX_LENGTH = 1 << 31     # PRAND_NOALLOC_MAX_LENGTH of include/prand.h
 
 
 def prand_free(state: int) -> None:

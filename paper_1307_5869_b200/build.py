@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libprand.so")
 MT_TABLE = os.path.join(HERE, "mt19937_polys.bin")
 SOURCES = ["prand.cu", "skip_ops.cpp", "k_lfsr113.cu", "k_mrg32k3a.cu", "k_mt19937.cu", "k_gmgq.cu",
-           "k_fill.cu", "k_devapi.cu", "k_probe.cu"]
+           "k_fill.cu", "k_devapi.cu", "k_probe.cu", "k_noalloc.cu"]
 HEADERS = ["internal.h", "k_common.cuh", "skip_ops.h"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

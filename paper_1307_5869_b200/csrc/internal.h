@@ -114,6 +114,11 @@ cudaError_t devapi_init_generate(cudaStream_t, int gen, const void *base, const 
 
 int sm_count();   // multiprocessor count of the current device
 
+// for entry points that live outside prand.cu: remember a failed CUDA call for prand_last_cuda_error (returns
+// PRAND_ERR_CUDA), add to the count behind prand_launch_count
+int record_cuda_error(cudaError_t e);
+void count_launches(unsigned n);
+
 // Test / tuning hooks.  One process-wide struct, filled ONCE from the PRAND_* environment variables the
 // first time the library needs it and changed afterwards only through prand_debug_set (prand.h): the
 // launch paths read plain fields, never the environment.

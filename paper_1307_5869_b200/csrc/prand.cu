@@ -788,6 +788,11 @@ extern "C" int prand_generate_f64_host(prand_state *st, double *out, uint64_t n,
     return generate_host(st, out, n, DT_F64, (cudaStream_t)s);
 }
 
+namespace prand {
+int record_cuda_error(cudaError_t e) { return cuda_fail(e); }
+void count_launches(unsigned n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+}  // namespace prand
+
 // ==================================================================================================
 // prand_generate_seq_* (SURVEY.md 8(f)1): PRAND's single-sequence array fill
 // ==================================================================================================
@@ -1199,6 +1204,7 @@ extern "C" const char *prand_strerror(int code)
     case PRAND_ERR_SIZE: return "byte count does not match prand_state_bytes()";
     case PRAND_ERR_ALLOC: return "allocation failed";
     case PRAND_ERR_INTERNAL: return "internal self-check failed";
+    case PRAND_ERR_CAPACITY: return "request exceeds the fixed capacity of the no-allocation entry point";
     default: return "unknown error code";
     }
 }
