@@ -473,8 +473,12 @@ template <int DT> cudaError_t dispatch_v(cudaStream_t stream, const GenArgs &a, 
     constexpr int VMAX = (DT == DT_F64) ? 2 : 4;   // one 128-bit store per row
     bool vec = (a.n_streams % VMAX == 0) && ((uintptr_t)a.out % 16 == 0);
     li->launches = 1;
-    if (vec) { li->kernel = (DT == DT_F64) ? "mrg32k3a_gen<V=2>" : "mrg32k3a_gen<V=4>"; return launch_gen<VMAX, DT>(stream, a); }
-    li->kernel = "mrg32k3a_gen<V=1>";
+    const bool hooked_int = DT != DT_F64 && debug_hooks().mrg_int;      // named apart so that a test can tell it ran
+    if (vec) {
+        li->kernel = (DT == DT_F64) ? "mrg32k3a_gen<V=2>" : hooked_int ? "mrg32k3a_gen<V=4,int>" : "mrg32k3a_gen<V=4>";
+        return launch_gen<VMAX, DT>(stream, a);
+    }
+    li->kernel = hooked_int ? "mrg32k3a_gen<V=1,int>" : "mrg32k3a_gen<V=1>";
     return launch_gen<1, DT>(stream, a);
 }
 

@@ -1413,9 +1413,14 @@ mt19937_wgen_kernel(const uint32_t *st_in, uint32_t *st_out, typename OutElem<DT
         const uint32_t *sp0 = staging + (lane & 1) * (WG_S * WG_CP) + h * WG_BOX + (lane >> 1);
         for (uint32_t u = par; u < turns; u += 2) {
             const uint32_t b = u % WG_NSB, tb = (u / 2) % WG_NTB;
-            // (all lanes poll and wait: no divergence to reconverge; only lane 0 has bulk groups pending)
+            // (all lanes poll the barrier: no divergence to reconverge)
             mbar_wait_sleep(sfull + 8 * b, (u / WG_NSB) & 1u);
-            if (u / 2 >= WG_NTB) asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(WG_NTB - 1) : "memory");
+            // bulk groups belong to the thread that committed them: lane 0 issued the stores, so lane 0 waits until the
+            // store that last used tile buffer tb has read it, and the warp barrier holds the other lanes' tile writes back
+            if (u / 2 >= WG_NTB) {
+                if (lane == 0) asm volatile("cp.async.bulk.wait_group.read %0;" :: "n"(WG_NTB - 1) : "memory");
+                __syncwarp();
+            }
             const uint32_t *sp = sp0 + b * SBUF;
             E *tp = my + tb * TILE + lane * 4;
 #pragma unroll

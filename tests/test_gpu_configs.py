@@ -95,6 +95,33 @@ def test_c3_mt19937_full_size_sampled():
     check_config(workloads.C3, 6)          # each sampled stream costs the oracle a 2^64-scale polynomial
 
 
+def test_c3_mt19937_every_output_equal_across_independent_kernels():
+    """C3 at full size (512 streams x 2^20): EVERY output and every final state of the default kernel (the
+    warp-per-stream cluster kernel with helper warps and TMA tile stores, 1638 turns of its staging ring) equals those of
+    the cluster-pair kernel (PRAND_MT_CFG=2: shared-memory window, plain stores), which shares none of the staging /
+    tile / TMA machinery.  The oracle pins sampled streams of this configuration (test above); this closes the rest
+    of the 2^29 numbers without oracle cost."""
+    w = workloads.C3
+    need_gpu(2 * w.out_bytes + (2 << 30))
+    outs, states, kernels = [], [], []
+    try:
+        for cfg in (None, "2"):
+            P.prand_debug_set("PRAND_MT_CFG", cfg)
+            g = P.Generator(w.gen, w.seed, w.n_streams, w.block_len)
+            out = torch.empty((w.n_per_stream, w.n_streams), dtype=TDT[w.dtype], device="cuda")
+            g.generate(w.n_per_stream, w.dtype, out=out)
+            torch.cuda.synchronize()
+            outs.append(out); states.append(g.state()); kernels.append(g.last_kernel)
+            g.close()
+    finally:
+        P.prand_debug_set("PRAND_MT_CFG", None)
+    assert kernels[0] == "mt19937_wgen<CS=2>" and kernels[1] != kernels[0], kernels
+    assert torch.equal(outs[0], outs[1]), f"{int((outs[0] != outs[1]).sum())} outputs differ between {kernels}"
+    assert states[0] == states[1]
+    del outs
+    torch.cuda.empty_cache()
+
+
 @pytest.mark.parametrize("w", workloads.C4, ids=lambda w: w.name)
 def test_c4_gm_f32_full_size_sampled(w):
     check_config(w, 24)

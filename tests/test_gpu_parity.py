@@ -7,6 +7,7 @@ fallback is never needed.  Small cases compare every output of every stream at s
 several thread groups / tiles with ragged tails; the BASELINE.json configurations run at full size in
 the launch configuration bench.py times and are compared on sampled streams (all rows of each).
 """
+import ctypes as C
 import os
 
 import numpy as np
@@ -107,7 +108,10 @@ def test_mt19937_every_kernel_configuration(cfg, monkeypatch):
                  (68, [1300, 1872], "u32"), (36, [5000], "f32"), (20, [3000, 6240], "f64")]
     if cfg >= 6:      # warp-per-stream cluster kernel: whole clusters of 8 streams
         cases = [(8, [624, 1248, 700, 4000], "u32"), (16, [2048], "f32"), (8, [1500, 625, 3121], "f64"),
-                 (72, [1300, 15, 1872, 656], "u32"), (40, [5000], "f32"), (24, [3000, 6240], "f64")]
+                 (72, [1300, 15, 1872, 656], "u32"), (40, [5000], "f32"), (24, [3000, 6240], "f64"),
+                 # > 20 turns of 640 rows in one call: the six staging buffers wrap three times and both tile buffers of
+                 # every helper warp are reused ten times (the wait for the TMA store that last read a tile), ragged tail
+                 (8, [640 * 21 + 333], "u32"), (16, [640 * 25 + 17, 640 * 13 + 1], "f64")]
     for ns, calls, dtype in cases:
         w = Workload(f"mt-cfg{cfg}", "mt19937", 5489, ns, 1000, sum(calls), dtype)
         got, st, kernel = lib_run(w, calls=calls)
@@ -149,8 +153,18 @@ def test_sub_section_chunking_changes_nothing(gen, monkeypatch):
     need_gpu()
     w = Workload("chunked", gen, workloads.SEED.get(gen, 1), 44, workloads.BLOCK_LEN[gen], 203, "f32")
     want, wst = oracle_run(w)
+    gid = P.gen_id(gen)
     for chunk in (4, 8, 52, 200):
         P.prand_debug_set("PRAND_CHUNK_LEN", str(chunk))
+        # the hook is in force: the launch policy cuts the first call's 150 rows into more than one sub-section
+        clen, ncs = C.c_uint64(), C.c_uint64()
+        assert P.lib().prand_host_plan(gid, w.n_streams, 150, 1, 148, C.byref(clen), C.byref(ncs)) == 0
+        gran = 32 if gen == "lfsr113" else 12
+        forced = -(-chunk // gran) * gran
+        if forced < 150:
+            assert clen.value == forced and ncs.value == -(-150 // forced) > 1, (clen.value, ncs.value)
+        else:                                             # (200: longer than either call, one section again)
+            assert ncs.value == 1
         got, st, _ = lib_run(w, calls=[150, 53])
         assert_same(w, got, want)
         assert st == wst
@@ -509,7 +523,8 @@ def test_mrg32k3a_integer_and_fp64_pipe_kernels_agree_with_the_oracle(dtype, mon
     for hook in (None, "1"):
         if hook:
             P.prand_debug_set("PRAND_MRG_INT", hook)
-        got, st, _ = lib_run(w, calls=[100, 103])
+        got, st, kernel = lib_run(w, calls=[100, 103])
+        assert kernel == ("mrg32k3a_gen<V=4,int>" if hook else "mrg32k3a_gen<V=4>"), kernel
         assert_same(w, got, want)
         assert st == wst
     P.prand_debug_set("PRAND_MRG_INT", None)
