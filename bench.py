@@ -13,9 +13,11 @@ block_len 2^76, 16,384 float64 per stream = 2^30 numbers, 8 GiB).  Prints ONE JS
   value      whole-job Gnumbers/s, device-resident output, max over ranks of the CUDA-event time
   e2e        same metric through prand_generate_<dtype>_host (pinned HOST buffer; device->host copies
              and the operator-table uploads inside the timed region)
-  roofline   generation kernel only: algorithmic output bytes / its mean CUDA-event duration inside
-             the timed steps, against MEASURED_PEAKS.json hbm_gbs; the fill-probe write peak of the
-             same run is reported beside it
+  roofline   generation kernel only: algorithmic bytes / its mean CUDA-event duration inside the timed steps,
+             against the largest write-capable rate measured (MEASURED_PEAKS.json hbm_gbs, the fill probe and
+             cudaMemsetAsync of the same run; the kernels only store, and stores alone beat the copy peak);
+             frac_of_copy_peak keeps the MEASURED_PEAKS figure; roofline.per_config = one short row per
+             configuration (kernel, ms, Gnumbers/s, bound, frac, instructions per number, oracle Gnumbers/s)
   cpu_baseline  the CPU oracle, as it stands, on all host cores, on a bounded sample of the workload
 
   per_config every other BASELINE.json configuration (C1, C3, C4 x2, C5 x9) and the paper's Table 7 task
@@ -50,6 +52,11 @@ ARITH = {"lfsr113": "u32", "mrg32k3a": "u32 (32x32->64 mul, mod 2^32-c) + f64 sc
 STATE_BYTES = {"lfsr113": 16, "mrg32k3a": 24, "mt19937": 2496, "gm19": 256, "gm29": 256, "gm31": 256,
                "gm55": 128, "gm61": 512, "gq58.1": 512, "gq58.3": 192, "gq58.4": 128}
 ALU_BOUND = {"gm19", "gm29", "gm31", "gm55", "gm61", "gq58.1", "gq58.3", "gq58.4"}
+# SURVEY.md 8(d) table, "Algorithmic integer work / number (estimate)": the planning figure the ncu count of a kernel
+# is read against (the alu `frac` is issue-slot utilisation of the kernel's OWN instruction count; it says how busy
+# the SM is, and only together with count <= estimate how close the kernel is to the algorithm's cost)
+SURVEY_INSTR_PER_NUMBER = {"gm19": "~290", "gm29": "~290", "gm31": "~320", "gm61": "650-800", "gm55": "~200",
+                           "gq58.4": "~200", "gq58.3": "~300", "gq58.1": "300-800"}
 
 
 def load_alu_counts():
@@ -198,8 +205,8 @@ def run_reference(args, w):
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": w.numbers / (value * 1e9) * 1e3,      # a full step of `config` at the sampled rate
-        "sample_wall_ms_per_step": wall / max(1, args.steps) * 1e3,
+        "ms_per_step": wall / max(1, args.steps) * 1e3,      # measured: one step = one bounded sample of `config`
+        "ms_per_step_extrapolated_full_config": w.numbers / (value * 1e9) * 1e3,   # all numbers of `config` at that rate
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": ARITH.get(w.gen, "u32/u64 modular"), "data": "synthetic",
         "config": config_of(w),
@@ -221,12 +228,25 @@ def config_of(w):
 
 
 # ---- our arm -----------------------------------------------------------------------------------------
-def roofline_of(w, kernel, k_ms, peak, peak_src, share=None, fill_gbs=None):
+def hbm_peak(peak, peak_src, fill_gbs=None, memset_gbs=None):
+    """Denominator of the HBM rows.  The generation kernels only store, and a pure-store stream can run faster than
+    the read+write copy MEASURED_PEAKS.json was taken with, so the peak is the LARGEST write-capable rate measured:
+    MEASURED_PEAKS hbm_gbs, the fill probe of this run, cudaMemsetAsync of this run (SURVEY.md 8(d) "Write peak")."""
+    cands = [(peak, peak_src)]
+    if fill_gbs:
+        cands.append((fill_gbs, "fill probe of this run (prand_fill_u32: one 128-bit st.global.cs per thread, CTAs in launch order)"))
+    if memset_gbs:
+        cands.append((memset_gbs, "cudaMemsetAsync of this run"))
+    return max(cands, key=lambda c: c[0])
+
+
+def roofline_of(w, kernel, k_ms, peak, peak_src, share=None, fill_gbs=None, memset_gbs=None):
     """The bench line's `roofline` object for one launch of `kernel` that took k_ms on workload w."""
     alg = algorithmic_bytes(w)
     out_gbs = w.out_bytes / (k_ms * 1e-3) / 1e9
     alg_gbs = alg / (k_ms * 1e-3) / 1e9
     traffic = load_traffic(kernel)
+    wpeak, wsrc = hbm_peak(peak, peak_src, fill_gbs, memset_gbs)
     if w.gen in ALU_BOUND:                         # integer-bound: report against the issue peak
         counts = load_alu_counts()
         ipn, src, pipes = counts.get(kernel, (None, None, {}))
@@ -235,16 +255,25 @@ def roofline_of(w, kernel, k_ms, peak, peak_src, share=None, fill_gbs=None):
         r = {"bound": "alu", "achieved": a_g, "peak": p_g, "unit": "Gthread-instr/s",
              "frac": a_g / p_g if a_g else None, "traffic": traffic, "kernel": kernel, "kernel_ms": k_ms,
              "thread_instr_per_number": ipn, "thread_instr_source": src, "ncu_pipe_pct": pipes,
+             "survey_estimate_instr_per_number": SURVEY_INSTR_PER_NUMBER.get(w.gen),
+             "frac_is": "issue-slot utilisation of the kernel's own ncu instruction count",
              "peak_source": "148 SMs x 4 schedulers x 32 lanes x sm_max_mhz (DESIGN.md 6.5, profiles/pipe_rates.md)",
-             "out_gbs": out_gbs, "hbm_peak_gbs": peak, "frac_of_hbm": alg_gbs / peak}
+             "out_gbs": out_gbs, "hbm_peak_gbs": wpeak, "frac_of_hbm": alg_gbs / wpeak}
     else:
-        r = {"bound": "hbm", "achieved": alg_gbs, "peak": peak, "unit": "GB/s", "frac": alg_gbs / peak,
+        r = {"bound": "hbm", "achieved": alg_gbs, "peak": wpeak, "unit": "GB/s", "frac": alg_gbs / wpeak,
              "traffic": traffic, "kernel": kernel, "kernel_ms": k_ms,
              "algorithmic_bytes_per_launch": alg, "out_bytes_per_launch": w.out_bytes, "out_gbs": out_gbs,
-             "peak_source": peak_src}
+             "peak_source": wsrc + " = the largest of the measured write-capable rates",
+             "copy_peak_gbs": peak, "copy_peak_source": peak_src, "frac_of_copy_peak": alg_gbs / peak}
         if fill_gbs:
             r["write_peak_same_run_gbs"] = fill_gbs
             r["frac_of_write_peak"] = alg_gbs / fill_gbs
+        if memset_gbs:
+            r["memset_write_peak_gbs"] = memset_gbs
+        # a kernel cannot beat the roofline: a fraction above 1 means the denominator is too low, not that the kernel is fast
+        if r["frac"] > 1.0:
+            raise SystemExit(f"bench.py: {w.name} {kernel}: {alg_gbs:.0f} GB/s exceeds the HBM peak {wpeak:.0f} GB/s "
+                             f"({wsrc}): the roofline denominator is too low")
     if share is not None:
         r["kernel_share_of_step"] = share
     return r
@@ -289,7 +318,8 @@ def launch_floor_us(torch, P):
             "back_to_back_us_per_launch": a.elapsed_time(b)}
 
 
-def time_config(torch, P, w, steps, warmup, flush, peak, peak_src, device_index=0):
+def time_config(torch, P, w, steps, warmup, flush, peak, peak_src, device_index=0, fill_gbs=None, memset_gbs=None,
+                cpu_seconds=0.0):
     """One per_config row: stream initialisation (wall clock around prand_init + synchronise, host
     operator preparation included) and the generation call alone (CUDA events, L2 flushed before each)."""
     tdt = {"u32": torch.int32, "f32": torch.float32, "f64": torch.float64}[w.dtype]
@@ -314,8 +344,15 @@ def time_config(torch, P, w, steps, warmup, flush, peak, peak_src, device_index=
     del out
     torch.cuda.empty_cache()
     med = statistics.median(gen_ms)
-    roof = roofline_of(w, kernel, med, peak, peak_src)
-    return {"workload": w.name, "gen": w.gen, "dtype": w.dtype, "n_streams": w.n_streams,
+    roof = roofline_of(w, kernel, med, peak, peak_src, fill_gbs=fill_gbs, memset_gbs=memset_gbs)
+    cpu = None
+    if cpu_seconds > 0:                     # SURVEY.md 8(d) "Oracle timing": the oracle on this configuration, same run
+        cores = os.cpu_count() or 1
+        v, sample = oracle_sample_rate(w, cpu_seconds, cores)
+        cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+    return {"cpu_baseline": cpu, "hbm_peak_gbs": roof.get("hbm_peak_gbs", roof["peak"]),
+            "survey_estimate_instr_per_number": roof.get("survey_estimate_instr_per_number"),
+            "workload": w.name, "gen": w.gen, "dtype": w.dtype, "n_streams": w.n_streams,
             "n_per_stream": w.n_per_stream, "api": name, "kernel": kernel, "launches_per_call": launches,
             "gen_ms": med, "gen_ms_best": min(gen_ms), "gnumbers_per_s": w.numbers / (med * 1e-3) / 1e9,
             "bound": roof["bound"], "frac": roof["frac"], "out_gbs": roof["out_gbs"],
@@ -502,8 +539,8 @@ def run_ours(args, w):
         return
     peak, peak_src = load_peaks()
     k_ms = statistics.mean(kernel_ms)
-    roofline = roofline_of(w, last_kernel[0], k_ms, peak, peak_src, share=k_ms / ms_per_step, fill_gbs=fill_gbs)
-    roofline["memset_write_peak_gbs"] = memset_gbs
+    roofline = roofline_of(w, last_kernel[0], k_ms, peak, peak_src, share=k_ms / ms_per_step, fill_gbs=fill_gbs,
+                           memset_gbs=memset_gbs)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
@@ -518,18 +555,34 @@ def run_ours(args, w):
         torch.cuda.empty_cache()
         line["launch_floor_us"] = launch_floor_us(torch, P)
         rows = []
+        if not args.no_cpu:
+            import oracle
+            oracle.build()
         for name in workloads.ALL:
             rows.append(time_config(torch, P, workloads.ALL[name], args.config_steps, 3, flush, peak, peak_src,
-                                    local_rank))
+                                    local_rank, fill_gbs=fill_gbs, memset_gbs=memset_gbs,
+                                    cpu_seconds=0.0 if args.no_cpu else 2.0))
             print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
         line["per_config"] = rows
+        # the same table in short form inside `roofline` (one row per generator / configuration of BASELINE.json)
+        roofline["per_config"] = {
+            r["workload"]: {"kernel": r["kernel"], "ms": round(r["gen_ms"], 5), "gnps": round(r["gnumbers_per_s"], 2),
+                            "bound": r["bound"], "frac": round(r["frac"], 4) if r["frac"] is not None else None,
+                            "instr_per_number": r["thread_instr_per_number"],
+                            "survey_instr_per_number": r["survey_estimate_instr_per_number"],
+                            "init_ms": round(r["init_ms"], 3),
+                            "cpu_gnps": round(r["cpu_baseline"]["value"], 4) if r["cpu_baseline"] else None}
+            for r in rows}
         line["jump_methods"] = jump_methods(torch, P)
+        line["pipe_rates"] = pipe_rates(torch, P, local_rank, calls=7)
         line["device_api"] = device_api_rates(torch, P)
         line["per_config_note"] = ("generation call alone (prand_generate_* / prand_generate_seq_*), CUDA-event median of "
                                    f"{args.config_steps} calls after 3 warm-ups, 256 MB written before each call (L2 flush); "
-                                   "frac: hbm = algorithmic bytes (output + 2 x state) / gen_ms / MEASURED_PEAKS hbm_gbs; "
+                                   "frac: hbm = algorithmic bytes (output + 2 x state) / gen_ms / the largest measured write-capable "
+                                   "rate (MEASURED_PEAKS hbm_gbs, fill probe, cudaMemsetAsync of this run); "
                                    "alu = ncu thread-instructions per number (profiles/alu_counts.csv) x numbers / gen_ms / "
-                                   "issue peak; init_ms = best wall time of prand_init + synchronise (3 runs)")
+                                   "issue peak; init_ms = best wall time of prand_init + synchronise (3 runs); cpu_baseline = the oracle on "
+                                   "a ~2 s sample of the same configuration, all host cores")
     if world == 1 and not args.no_cpu:
         import oracle
         oracle.build()
@@ -553,7 +606,8 @@ def run_sweep(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     rows = []
     for name in names:
-        rows.append(time_config(torch, P, workloads.ALL[name], args.steps, args.warmup, flush, peak, peak_src))
+        rows.append(time_config(torch, P, workloads.ALL[name], args.steps, args.warmup, flush, peak, peak_src,
+                                fill_gbs=fill_gbs, memset_gbs=memset_gbs))
         print(json.dumps(rows[-1]), file=sys.stderr, flush=True)
     result = {"write_peak_gbs": fill_gbs, "memset_write_peak_gbs": memset_gbs, "hbm_copy_peak_gbs": peak,
               "launch_floor_us": launch_floor_us(torch, P), "rows": rows}
@@ -563,49 +617,31 @@ def run_sweep(args):
 
 
 # ---- instruction rates of the SM pipes (profiles/pipe_rates.md) ----------------------------------------
-def run_pipe_rates(args):
-    import torch
-    import paper_1307_5869_b200 as P
-
-    torch.cuda.set_device(0)
-    sms = torch.cuda.get_device_properties(0).multi_processor_count
+def pipe_rates(torch, P, device_index=0, calls=15):
+    """Dependent-free instruction-rate probes (prand_probe_pipe): thread-level operations per clock per SM at the SM
+    clock read while they run -- confirms the issue peak the alu rows are divided by."""
+    sms = torch.cuda.get_device_properties(device_index).multi_processor_count
     rows = []
     for op, name in enumerate(P.prand_probe_pipe_names()):
         ops = [0]
 
         def fn(op=op):
             ops[0] = P.prand_probe_pipe(op, 2000)
-        with ClockSampler(0, period_s=0.001) as clk:
-            ms = event_ms(torch, fn, 15, warm=3)
+        with ClockSampler(device_index, period_s=0.001) as clk:
+            ms = event_ms(torch, fn, calls, warm=3)
         mhz = clk.summary()["sm_mhz"] or 1965.0
         med = statistics.median(ms)
         rows.append({"op": name, "ms": med, "thread_ops": ops[0], "sm_mhz": mhz,
                      "ops_per_clk_per_sm": ops[0] / (med * 1e-3) / (mhz * 1e6) / sms})
-    print(json.dumps({"pipe_rates": rows, "sms": sms}), flush=True)
+    return {"pipe_rates": rows, "sms": sms}
 
 
-# ---- store pieces of few-stream kernels (profiles/r02_store_pieces.md) -------------------------------------
-def run_store_probe(args):
-    """2^20 rows of 2048 bytes (C3's output) written as 16-byte pieces by 128 CTAs resp. 32-byte pieces by 64 CTAs,
-    with STG and with TMA tensor stores, and how the time grows when partner CTAs start `skew` clocks apart."""
+def run_pipe_rates(args):
     import torch
     import paper_1307_5869_b200 as P
 
     torch.cuda.set_device(0)
-    rows = (1 << 20) // 160 * 160
-    buf = torch.empty(rows * 2048, dtype=torch.uint8, device="cuda")
-    out = []
-    for method, mname in ((0, "stg"), (1, "tma")):
-        for pb, g in ((16, 128), (32, 64), (64, 32)):
-            for mode in (0, 1, 2, 3):
-                for skew in ((0,) if mode == 0 else (500, 2000, 10000, 50000)):
-                    def fn():
-                        P.prand_probe_store_pieces(buf.data_ptr(), buf.numel(), method, pb, g, rows, skew, mode)
-                    ms = statistics.median(event_ms(torch, fn, 5, warm=2))
-                    delay_ms = {0: 0, 1: 1, 2: 7, 3: 3}[mode] * skew / 1.965e6
-                    out.append({"method": mname, "piece_bytes": pb, "ctas": g, "skew_mode": mode, "skew_clocks": skew,
-                                "ms": ms, "ms_net_of_start_delay": ms - delay_ms, "gbs": rows * 2048 / (ms - delay_ms) / 1e6})
-    print(json.dumps({"store_pieces": out, "rows": rows, "row_bytes": 2048}), flush=True)
+    print(json.dumps(pipe_rates(torch, P)), flush=True)
 
 
 def main():
@@ -620,17 +656,14 @@ def main():
     ap.add_argument("--sweep", default=None, metavar="OUT.json", help="time every workload, write a table")
     ap.add_argument("--sweep-workloads", default=None, help="comma-separated workload names for --sweep")
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config table (all other configs)")
-    ap.add_argument("--config-steps", type=int, default=10, help="timed calls per per_config row")
+    ap.add_argument("--config-steps", type=int, default=20, help="timed calls per per_config row (SURVEY.md 8(d): >= 20)")
     ap.add_argument("--pipe-rates", action="store_true", help="print the SM pipe instruction rates (probe kernels)")
-    ap.add_argument("--store-probe", action="store_true", help="print the store-piece probe table (profiles/r02_store_pieces.md)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours" and not args.sweep:
         args.warmup = 3                          # timing rule: at least three warm-up steps
     w = workloads.ALL[args.workload]
     if args.pipe_rates:
         return run_pipe_rates(args)
-    if args.store_probe:
-        return run_store_probe(args)
     if args.sweep:
         return run_sweep(args)
     if args.impl == "reference":

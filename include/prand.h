@@ -291,21 +291,12 @@ int prand_fill_u32(uint32_t *out, uint64_t n_words, uint32_t value, void *cuda_s
  *                       pointer) receives the thread-level operations one launch executes, so that
  *                       thread_ops / (time x SM clock x SM count) = operations per clock per SM
  *                       (profiles/pipe_rates.md).
- *   prand_probe_store_pieces  the store pattern of a kernel that holds few streams per CTA: n_ctas CTAs each
- *                       write one piece of piece_bytes (16, 32 or 64) of every one of `rows` rows of the
- *                       [rows x n_ctas * piece_bytes] array at DEVICE pointer d_buf (buf_bytes large, 16-byte
- *                       aligned), method 0 = STG (4 bytes per lane), 1 = TMA tensor stores of [160 rows x piece]
- *                       boxes; CTA b starts skew_clocks late by skew_mode (0 none, 1 every second CTA, 2 (b mod
- *                       8) * skew, 3 sector pairs together, (pair mod 4) * skew): how far partner CTAs may drift
- *                       before partial-sector stores stop merging in L2 (profiles/r02_store_pieces.md).
  */
 int prand_probe_empty(void *cuda_stream);
 int prand_probe_memset(void *d_ptr, int value, size_t bytes, void *cuda_stream);
 int prand_probe_pipe_count(void);
 const char *prand_probe_pipe_name(int op);
 int prand_probe_pipe(int op, uint64_t iters, uint64_t *thread_ops, void *cuda_stream);
-int prand_probe_store_pieces(void *d_buf, size_t buf_bytes, int method, int piece_bytes, int n_ctas, uint64_t rows,
-                             uint64_t skew_clocks, int skew_mode, void *cuda_stream);
 
 /*
  * prand_debug_set -- test / tuning hooks that select alternate kernels or algorithms; results never

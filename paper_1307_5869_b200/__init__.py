@@ -60,8 +60,6 @@ _SIGS = {
     "prand_probe_pipe_count": (C.c_int, []),
     "prand_probe_pipe_name": (C.c_char_p, [C.c_int]),
     "prand_probe_pipe": (C.c_int, [C.c_int, C.c_uint64, C.POINTER(C.c_uint64), C.c_void_p]),
-    "prand_probe_store_pieces": (C.c_int, [C.c_void_p, C.c_size_t, C.c_int, C.c_int, C.c_int, C.c_uint64, C.c_uint64, C.c_int,
-                                           C.c_void_p]),
     "prand_debug_set": (C.c_int, [C.c_char_p, C.c_char_p]),
     "prand_trim": (C.c_int, []),
     "prand_launch_count": (C.c_uint64, []),
@@ -231,12 +229,6 @@ def prand_probe_pipe(op: int, iters: int, stream=None) -> int:
     n = C.c_uint64()
     _check(lib().prand_probe_pipe(op, iters, C.byref(n), _stream_ptr(stream)), "prand_probe_pipe")
     return n.value
-
-
-def prand_probe_store_pieces(ptr: int, nbytes: int, method: int, piece_bytes: int, n_ctas: int, rows: int,
-                             skew_clocks: int = 0, skew_mode: int = 0, stream=None) -> None:
-    _check(lib().prand_probe_store_pieces(ptr, nbytes, method, piece_bytes, n_ctas, rows, skew_clocks, skew_mode,
-                                          _stream_ptr(stream)), "prand_probe_store_pieces")
 
 
 def prand_probe_pipe_names() -> list[str]:

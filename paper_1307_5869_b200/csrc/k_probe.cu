@@ -7,7 +7,6 @@
 // PTX, so that the SASS opcode is the intended one -- checked with `cuobjdump -sass`, see
 // profiles/pipe_rates.md) for `iters` iterations; the grid is 8 CTAs x 256 threads per SM, i.e. the
 // scheduler always has an eligible warp.  thread-ops / (time x SM clock x SMs) = ops per clock per SM.
-#include <cuda.h>                                         // CUtensorMap (types only: the encoder comes through the runtime)
 #include "k_common.cuh"
 
 namespace prand {
@@ -93,59 +92,6 @@ pipe_kernel(uint32_t *sink, uint64_t iters, uint32_t b, uint32_t c)
     if (r == 0x12345u && sink) sink[0] = r;                 // keeps the chains alive
 }
 
-
-// ---- store-piece probe (profiles/r02_store_pieces.md) ----------------------------------------------------
-// What the few-stream MT19937 kernels are up against: G CTAs (one per SM) each own one piece of PB bytes of every
-// row of a [rows x G * PB bytes] array -- C3's geometry is G = 128, PB = 16 -- and write all rows, either with
-// STG (4 bytes per lane, PB / 4 adjacent lanes per row) or with TMA tensor stores of [160 rows x PB bytes] boxes
-// issued by one thread.  CTA b starts `skew` clocks late according to skew_mode: 1 = every second CTA (the two
-// halves of a 32-byte sector drift apart), 2 = (b mod 8) * skew (the pieces of a 128-byte line drift apart),
-// 3 = sector pairs stay together, pair p is (p mod 4) * skew late.
-__device__ __forceinline__ void probe_delay(uint64_t skew, int skew_mode)
-{
-    const unsigned b = blockIdx.x;
-    const uint64_t d = skew_mode == 1 ? (b & 1u) * skew : skew_mode == 2 ? (b % 8u) * skew : skew_mode == 3 ? ((b / 2u) % 4u) * skew : 0;
-    const long long t0 = clock64();
-    while ((uint64_t)(clock64() - t0) < d) { }
-}
-
-__global__ void __launch_bounds__(1024)
-store_stg_kernel(char *out, uint64_t pitch, uint64_t rows, int pb, uint64_t skew, int skew_mode)
-{
-    probe_delay(skew, skew_mode);
-    const int lp = pb / 4, tid = threadIdx.x, nt = blockDim.x;
-    const uint64_t col = (uint64_t)blockIdx.x * pb + (uint64_t)(tid % lp) * 4;
-    for (uint64_t r = tid / lp; r < rows; r += nt / lp)
-        __stcs(reinterpret_cast<uint32_t *>(out + r * pitch + col), (uint32_t)tid);
-}
-
-constexpr int PROBE_BOX = 160;
-
-__global__ void __launch_bounds__(32)
-store_tma_kernel(const __grid_constant__ CUtensorMap tmap, uint64_t rows, int words, uint64_t skew, int skew_mode)
-{
-    extern __shared__ __align__(128) uint32_t probe_tile[];
-    for (int i = threadIdx.x; i < PROBE_BOX * words; i += blockDim.x) probe_tile[i] = i * 2654435761u;
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        probe_delay(skew, skew_mode);
-        const uint32_t src = (uint32_t)__cvta_generic_to_shared(probe_tile);
-        const int x = blockIdx.x * words;
-        for (uint64_t r = 0; r + PROBE_BOX <= rows; r += PROBE_BOX) {
-            asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
-                         :: "l"(&tmap), "r"(x), "r"((int)r), "r"(src) : "memory");
-            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-            asm volatile("cp.async.bulk.wait_group.read 4;" ::: "memory");
-        }
-        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
-    }
-}
-
-typedef CUresult (*ProbeEncodeFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
-                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
 template <int OP> cudaError_t launch_pipe(cudaStream_t stream, unsigned blocks, uint64_t iters)
 {
     pipe_kernel<OP><<<blocks, 256, 0, stream>>>(nullptr, iters, 0x9E3779B9u, 0x7F4A7C15u);
@@ -191,38 +137,4 @@ extern "C" int prand_probe_pipe(int op, uint64_t iters, uint64_t *thread_ops, vo
     default: return PRAND_ERR_ARG;
     }
     return e == cudaSuccess ? PRAND_OK : PRAND_ERR_CUDA;
-}
-
-extern "C" int prand_probe_store_pieces(void *d_buf, size_t buf_bytes, int method, int piece_bytes, int n_ctas, uint64_t rows,
-                                        uint64_t skew_clocks, int skew_mode, void *cuda_stream)
-{
-    if (!d_buf || (method != 0 && method != 1) || (piece_bytes != 16 && piece_bytes != 32 && piece_bytes != 64) || n_ctas <= 0 ||
-        rows == 0 || rows >= (1ull << 31) || skew_mode < 0 || skew_mode > 3 || (uintptr_t)d_buf % 16 != 0)
-        return PRAND_ERR_ARG;
-    const uint64_t pitch = (uint64_t)n_ctas * piece_bytes;
-    if (pitch * rows > buf_bytes) return PRAND_ERR_ARG;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
-    if (method == 0) {
-        store_stg_kernel<<<(unsigned)n_ctas, 1024, 0, s>>>((char *)d_buf, pitch, rows, piece_bytes, skew_clocks, skew_mode);
-        return cudaGetLastError() == cudaSuccess ? PRAND_OK : PRAND_ERR_CUDA;
-    }
-    static ProbeEncodeFn encode = [] {
-        void *p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
-            p = nullptr;
-        return (ProbeEncodeFn)p;
-    }();
-    if (!encode) return PRAND_ERR_CUDA;
-    const int words = piece_bytes / 4;
-    CUtensorMap tm;
-    const cuuint64_t dims[2] = {(cuuint64_t)n_ctas * words, rows};
-    const cuuint64_t strides[1] = {pitch};
-    const cuuint32_t box[2] = {(cuuint32_t)words, PROBE_BOX};
-    const cuuint32_t es[2] = {1, 1};
-    if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, d_buf, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return PRAND_ERR_CUDA;
-    store_tma_kernel<<<(unsigned)n_ctas, 32, PROBE_BOX * piece_bytes, s>>>(tm, rows, words, skew_clocks, skew_mode);
-    return cudaGetLastError() == cudaSuccess ? PRAND_OK : PRAND_ERR_CUDA;
 }

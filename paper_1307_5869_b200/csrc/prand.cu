@@ -610,10 +610,22 @@ void plan_chunks(int gen, uint64_t ns, uint64_t n, int dtype, int sms, uint64_t 
         // one balanced wave: as many equal chunks as fit the threads resident at once, never more
         // (a second, partial wave would cost a whole chunk time)
         const uint64_t capacity = (uint64_t)sms * 1024;
-        if (2 * threads > capacity) return;
-        const uint64_t want = capacity / threads;
-        len = (n + want - 1) / want;
-        if (len < min_len) len = min_len;
+        // the store-bound kernels (LFSR113, MRG32K3A with 8-byte outputs) are the exception: measured on B200, sub-sections
+        // of about 1024 rows in several waves beat one wave of long ones (C2: 4 x 4096 rows 1.379 ms, 16 x 1024 rows
+        // 1.294 ms; C5-lfsr113: unchunked 1.341 ms, 2 x 1024 rows 1.301 ms) -- CTAs are handed out in index order, so the
+        // rows being written at any moment stay close together in DRAM, and a retiring CTA is replaced at once; below
+        // ~512 rows the jump to a sub-section's start costs more than that gains
+        const bool store_bound = gen == PRAND_LFSR113 || (gen == PRAND_MRG32K3A && dtype == DT_F64);
+        const uint64_t wave_len = 1024;
+        if (2 * threads > capacity) {
+            if (!store_bound || n < 2 * wave_len) return;
+            len = wave_len;
+        } else {
+            const uint64_t want = capacity / threads;
+            len = (n + want - 1) / want;
+            if (len < min_len) len = min_len;
+            if (store_bound && len > wave_len) len = wave_len;
+        }
     }
     // whole row blocks per chunk: 32 for LFSR113's bit-stream form, else 12 (4: row groups of the
     // 4-lane GM path; 3: MRG32K3A's renamed rotation)

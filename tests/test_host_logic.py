@@ -52,7 +52,7 @@ def test_library_exports_every_declared_symbol():
 def test_version_and_strerror():
     assert b"sm_100a" in P.lib().prand_version()
     assert P.lib().prand_strerror(0) == b"ok"
-    for code in range(-8, 0):
+    for code in range(-9, 0):
         assert P.lib().prand_strerror(code) not in (b"ok", b"unknown error code")
 
 
@@ -188,14 +188,21 @@ def test_plan_covers_all_rows(gen):
                 assert (nc - 1) * cl < n <= nc * cl
                 if nc > 1:
                     assert cl % 4 == 0 and gen != "mt19937"
-    # enough streams: never chunk
-    assert P.prand_host_plan("lfsr113", 2**20, 2048, "u32", 148) == (2048, 1)
+    # enough streams and an integer-bound kernel: never chunk
+    assert P.prand_host_plan("gm31", 2**20, 2048, "u32", 148) == (2048, 1)
+    assert P.prand_host_plan("mrg32k3a", 2**20, 2048, "u32", 148) == (2048, 1)
+    # the store-bound kernels (LFSR113, MRG32K3A f64) take sub-sections of 1024 rows in several waves (measured faster
+    # than one wave of long ones), also when the streams alone would fill the GPU; short calls stay whole
+    assert P.prand_host_plan("lfsr113", 2**20, 2048, "u32", 148) == (1024, 2)
+    assert P.prand_host_plan("lfsr113", 2**20, 2047, "u32", 148) == (2047, 1)
+    assert P.prand_host_plan("mrg32k3a", 65536, 16384, "f64", 148) == (1032, 16)       # C2 (whole groups of 12 rows)
+    assert P.prand_host_plan("lfsr113", 1024, 2**20, "u32", 148) == (1024, 1024)
     # config 1 (1024 streams x 4096) must be cut to fill the GPU: small L2-resident outputs run one stream per
     # thread, so 1024 threads x 64 sub-sections of 64 rows (a second wave would cost a whole sub-section)
     assert P.prand_host_plan("lfsr113", 1024, 4096, "u32", 148) == (64, 64)
-    # the same streams with long rows (output beyond 64 MiB): four streams per thread, sub-sections fill 148 x 1024 threads
-    cl, nc = P.prand_host_plan("lfsr113", 1024, 2**20, "u32", 148)
-    assert nc * (1024 // 4) <= 148 * 1024 < 2 * nc * (1024 // 4) and cl % 32 == 0
+    # integer-bound generators keep one balanced wave: sub-sections fill 148 x 1024 threads, no more
+    cl, nc = P.prand_host_plan("gm31", 1024, 2**20, "u32", 148)
+    assert nc * 1024 <= 148 * 1024 < 2 * nc * 1024 and cl % 4 == 0
 
 
 def test_section_plan_covers_the_array_exactly_once():
