@@ -69,6 +69,10 @@ int prand_host_gm_kq(int gen, uint64_t mant, unsigned log2, uint64_t *k_n, uint6
  * cut into n_sections sections of sec_len (a multiple of 32; the last one may be shorter).
  */
 int prand_host_plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec_len);
+/* The plan above is the one of a device with 148 multiprocessors (B200).  prand_generate_seq_* plans with the
+ * multiprocessor count of the device it runs on (MT19937 takes at most 4 sections per multiprocessor); this variant
+ * takes that count, so that the cuts can be located on any device. */
+int prand_host_plan_sections_sm(int gen, uint64_t length, int sm_count, uint64_t *n_sections, uint64_t *sec_len);
 
 #ifdef __cplusplus
 }

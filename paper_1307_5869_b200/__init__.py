@@ -79,6 +79,7 @@ _SIGS = {
     "prand_host_mt19937_table": (C.c_int, [C.c_uint64, C.c_uint, C.c_void_p]),
     "prand_host_gm_kq": (C.c_int, [C.c_int, C.c_uint64, C.c_uint, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
     "prand_host_plan_sections": (C.c_int, [C.c_int, C.c_uint64, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
+    "prand_host_plan_sections_sm": (C.c_int, [C.c_int, C.c_uint64, C.c_int, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
     "prand_host_plan": (C.c_int, [C.c_int, C.c_uint64, C.c_uint64, C.c_int, C.c_int,
                                   C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]),
 }

@@ -1315,6 +1315,14 @@ extern "C" int prand_host_plan_sections(int gen, uint64_t length, uint64_t *n_se
     return PRAND_OK;
 }
 
+extern "C" int prand_host_plan_sections_sm(int gen, uint64_t length, int sm_count, uint64_t *n_sections, uint64_t *sec_len)
+{
+    if (gen < 0 || gen >= PRAND_NGEN) return PRAND_ERR_GEN;
+    if (!n_sections || !sec_len || length == 0 || sm_count <= 0) return PRAND_ERR_ARG;
+    plan_sections(gen, length, n_sections, sec_len, sm_count);
+    return PRAND_OK;
+}
+
 extern "C" int prand_host_plan(int gen, uint64_t n_streams, uint64_t n_per_stream, int dtype, int sms,
                                uint64_t *chunk_len, uint64_t *n_chunks)
 {

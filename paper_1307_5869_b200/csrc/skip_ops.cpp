@@ -403,6 +403,36 @@ std::string table_path()
     }
     return "mt19937_polys.bin";
 }
+// A table of the right size can still be stale (another record layout) or damaged, and would silently give wrong
+// block-split streams.  Every record is the square of its predecessor in its chain (x^(2^n); x^(m 2^i) for each m), the
+// chains meet at x^16 = record (m = 16, i = 0) = record (2^4), and x^m is a product of the first records: checking the
+// head, some middle links and the tail of every chain with the host's own polynomial arithmetic costs ~50 squarings
+// once per process and catches a wrong layout, a truncated-and-padded file and most bit damage.
+bool table_consistent(const std::vector<MtPoly> &t)
+{
+    auto same = [](const MtPoly &a, const MtPoly &b) { return std::memcmp(a.w, b.w, sizeof a.w) == 0; };
+    MtPoly r;
+    for (int n : {1, 2, 3, 4, 17, 100, 255, 256, MT_TABLE_POW2 - 1}) {
+        mt19937_sqrmod(r, t[n - 1]);
+        if (!same(r, t[n])) return false;
+    }
+    for (int m = MT_TABLE_M0; m <= MT_TABLE_M1; m++) {
+        const MtPoly *row = t.data() + MT_TABLE_POW2 + (m - MT_TABLE_M0) * MT_TABLE_SHIFTS;
+        MtPoly xm;                                            // x^m from the bits of m
+        bool first = true;
+        for (int b = 0; b < 5; b++) {
+            if (!((m >> b) & 1)) continue;
+            if (first) { xm = t[b]; first = false; }
+            else mt19937_mulmod(xm, xm, t[b]);
+        }
+        if (!same(xm, row[0])) return false;
+        for (int i : {1, 64, MT_TABLE_SHIFTS - 1}) {
+            mt19937_sqrmod(r, row[i - 1]);
+            if (!same(r, row[i])) return false;
+        }
+    }
+    return true;
+}
 }  // namespace
 
 const MtPoly *mt19937_table()
@@ -418,7 +448,11 @@ const MtPoly *mt19937_table()
             const bool exact = n == t.size() && std::fread(&extra, 1, 1, f) == 0;
             std::fclose(f);
             // record 0 must be the polynomial x, record 1 x^2: a cheap guard against a foreign file
-            if (exact && t[0].w[0] == 2 && t[1].w[0] == 4) g_table.swap(t);
+            if (exact && t[0].w[0] == 2 && t[1].w[0] == 4) {
+                if (table_consistent(t)) g_table.swap(t);
+                else std::fprintf(stderr, "libprand: %s fails its consistency check (stale or damaged file); MT19937 jump "
+                                          "polynomials are computed on the host instead\n", table_path().c_str());
+            }
         }
     }
     return g_table.empty() ? nullptr : g_table.data();

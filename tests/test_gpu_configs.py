@@ -148,7 +148,8 @@ def test_t7_sequence_fill_full_size_sampled_sections(w):
     need_gpu(w.out_bytes + (6 << 30))
     n = w.n_per_stream
     S, L = C.c_uint64(), C.c_uint64()
-    assert P.lib().prand_host_plan_sections(P.gen_id(w.gen), n, C.byref(S), C.byref(L)) == 0
+    sms = torch.cuda.get_device_properties(0).multi_processor_count        # the plan of the device the fill runs on
+    assert P.lib().prand_host_plan_sections_sm(P.gen_id(w.gen), n, sms, C.byref(S), C.byref(L)) == 0
     S, L = S.value, L.value
     assert S > 16 and (S - 1) * L < n <= S * L
     g = P.Generator(w.gen, w.seed, 1, 0)

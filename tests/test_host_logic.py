@@ -217,6 +217,46 @@ def test_section_plan_covers_the_array_exactly_once():
             assert (S - 1) * L < length <= S * L
             assert S <= (4 * 148 if gen == "mt19937" else 131072)    # MT19937: one CTA of four sections per SM
     assert P.lib().prand_host_plan_sections(0, 0, C.byref(C.c_uint64()), C.byref(C.c_uint64())) == -2
+    # the plan of a device with another multiprocessor count (MT19937: four sections per multiprocessor)
+    S, L = C.c_uint64(), C.c_uint64()
+    for sms in (148, 132, 20):
+        assert P.lib().prand_host_plan_sections_sm(P.gen_id("mt19937"), 2**29, sms, C.byref(S), C.byref(L)) == 0
+        assert S.value <= 4 * sms < S.value + 4 and L.value % 32 == 0 and (S.value - 1) * L.value < 2**29 <= S.value * L.value
+    a, b = C.c_uint64(), C.c_uint64()
+    assert P.lib().prand_host_plan_sections(P.gen_id("mt19937"), 2**29, C.byref(a), C.byref(b)) == 0
+    assert P.lib().prand_host_plan_sections_sm(P.gen_id("mt19937"), 2**29, 148, C.byref(S), C.byref(L)) == 0
+    assert (a.value, b.value) == (S.value, L.value)
+    assert P.lib().prand_host_plan_sections_sm(0, 100, 0, C.byref(S), C.byref(L)) == -2
+
+
+def test_mt19937_table_file_is_checked_when_it_is_loaded(tmp_path):
+    """A table file of the right size whose records are not what they should be (stale layout, damaged bytes) must not
+    be used: the library checks chain links with its own polynomial arithmetic at load and falls back to host
+    arithmetic.  One process per case: the table is loaded once."""
+    import subprocess
+    import sys
+    good = os.path.join(os.path.dirname(P.LIB_PATH), "mt19937_polys.bin")
+    raw = bytearray(open(good, "rb").read())
+    assert len(raw) == 1792 * 2496
+    cases = {"good": bytes(raw)}
+    flipped = bytearray(raw); flipped[255 * 2496 + 1000] ^= 0x10          # one bit in record x^(2^255)
+    cases["bit flipped in a checked record"] = bytes(flipped)
+    shifted = bytearray(raw); shifted[2 * 2496:] = raw[3 * 2496:] + raw[2 * 2496:3 * 2496]   # records from 2 on moved up by one
+    cases["records shifted"] = bytes(shifted)
+    rows = bytearray(raw); rows[512 * 2496:(512 + 128) * 2496] = raw[(512 + 128) * 2496:(512 + 256) * 2496]   # row m=15 holds m=16's
+    cases["a row of another m"] = bytes(rows)
+    code = ("import paper_1307_5869_b200 as P; "
+            "print('TABLE', P.prand_host_mt19937_table(1 << 300) is not None, P.prand_host_mt19937_table(15 << 100) is not None)")
+    for name, data in cases.items():
+        path = tmp_path / "table.bin"
+        path.write_bytes(data)
+        env = dict(os.environ, PRAND_MT_TABLE=str(path), PYTHONPATH=ROOT)
+        r = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
+        assert r.returncode == 0, r.stderr
+        used = "TABLE True True" in r.stdout
+        assert used == (name == "good"), (name, r.stdout, r.stderr)
+        if name != "good":
+            assert "consistency check" in r.stderr
 
 
 def test_bench_reference_arm_prints_the_contract_line():
