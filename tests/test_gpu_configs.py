@@ -4,7 +4,9 @@ The oracle cannot produce 2^30 numbers in seconds, but every stream is defined b
 (stream s = base sequence advanced s * block_len), so it can compute any single
 stream on its own: each test generates the whole configuration on the GPU and compares ALL rows of a
 sample of streams (first, last, around CTA / warp boundaries, seeded random ones) plus the exported
-final states of those streams, bit for bit.  C1 is small enough to compare completely.
+final states of those streams, bit for bit.  C1, C2, C4-gm31, C5-lfsr113 and C5-mrg32k3a are compared COMPLETELY
+(every output, every final state, in column blocks); at C3 size every output of the default MT19937 kernel is also
+compared with an independent kernel's.
 """
 import ctypes as C
 import os
@@ -57,7 +59,7 @@ def check_config(w, n_sample):
     got = out.index_select(1, idx).cpu().numpy().view(NPDT[w.dtype])
     del out
     sb = oracle.state_bytes(w.gen)
-    states = g.state() if state_bytes <= (1 << 30) else None
+    states = g.state() if state_bytes <= (4 << 30) else None       # (C5-mt19937: 2.6 GB of windows)
     kernel = g.last_kernel
     g.close()
     torch.cuda.empty_cache()
@@ -71,6 +73,45 @@ def check_config(w, n_sample):
                                  f"row {i}: got {got[i, j]!r} want {want[i, 0]!r}")
         if states is not None:
             assert states[s * sb:(s + 1) * sb] == wst.tobytes(), f"{w.name} stream {s}: final state differs"
+
+
+def check_config_complete(w, block):
+    """EVERY output and EVERY final state of configuration w against the oracle, in column blocks of `block` streams
+    (the oracle computes any block of streams by position; all host cores).  SURVEY.md 8(c) "Verification volume"."""
+    state_bytes = w.n_streams * oracle.state_bytes(w.gen)
+    need_gpu(w.out_bytes + 3 * state_bytes + (2 << 30))
+    g = P.Generator(w.gen, w.seed, w.n_streams, w.block_len)
+    out = torch.empty((w.n_per_stream, w.n_streams), dtype=TDT[w.dtype], device="cuda")
+    g.generate(w.n_per_stream, w.dtype, out=out)
+    torch.cuda.synchronize()
+    states, kernel = g.state(), g.last_kernel
+    g.close()
+    sb = oracle.state_bytes(w.gen)
+    for s0 in range(0, w.n_streams, block):
+        nb = min(block, w.n_streams - s0)
+        got = out[:, s0:s0 + nb].contiguous().cpu().numpy().view(BITS[w.dtype])
+        want, wst = oracle.streams(w.gen, w.seed, s0, nb, w.block_len, w.n_per_stream, w.dtype, threads=CPU_THREADS)
+        wb = np.ascontiguousarray(want).view(BITS[w.dtype])
+        if not np.array_equal(got, wb):
+            i, j = np.argwhere(got != wb)[0]
+            raise AssertionError(f"{w.name} [{kernel}]: {(got != wb).sum()} outputs of streams {s0}..{s0 + nb - 1} differ; "
+                                 f"first at row {i} stream {s0 + j}: got {got[i, j]:#x} want {wb[i, j]:#x}")
+        assert states[s0 * sb:(s0 + nb) * sb] == wst.tobytes(), f"{w.name}: final states of streams {s0}.. differ"
+    del out
+    torch.cuda.empty_cache()
+
+
+COMPLETE = [(workloads.C2, 4096), (workloads.ALL["C5-lfsr113"], 65536), (workloads.ALL["C5-mrg32k3a"], 65536),
+            (workloads.ALL["C4-gm31"], 16384)]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("w,block", COMPLETE, ids=lambda x: getattr(x, "name", str(x)))
+def test_full_size_every_output_and_state(w, block):
+    """The exactness arguments of the fast kernels are rare-event claims (MRG32K3A's second component on the FP64 pipe,
+    GM31's 14 points in double precision, the estimate-and-correct reductions): where the oracle affords it the whole
+    configuration is compared, all 2^30 / 2^31 numbers and all final states, not a sample."""
+    check_config_complete(w, block)
 
 
 def test_c1_lfsr113_complete():
@@ -129,7 +170,8 @@ def test_c4_gm_f32_full_size_sampled(w):
 
 @pytest.mark.parametrize("w", workloads.C5, ids=lambda w: w.name)
 def test_c5_sweep_full_size_sampled(w):
-    check_config(w, 6 if w.gen == "mt19937" else 40)
+    # (LFSR113 and MRG32K3A are compared completely above; the GM/GQ generators on >= 1024 streams)
+    check_config(w, 6 if w.gen == "mt19937" else 1024 if w.gen.startswith("g") else 40)
 
 
 # in-place sequence fills beside the paper's two: a ragged length that leaves the last section short (and the last
