@@ -305,7 +305,8 @@ int prand_probe_pipe(int op, uint64_t iters, uint64_t *thread_ops, void *cuda_st
  *   (value NULL or "" restores the default).  Names: PRAND_MT_CFG (0..6: MT19937 generation kernel),
  *   PRAND_MT_APPLY (list, win, win2, win4, multi: other polynomial-application kernels), PRAND_GM_LP (1, 2, 4), PRAND_GM31_NF (0, 10, 12, 14, 16), PRAND_GM_WATCH,
  *   PRAND_MRG_INT, PRAND_GM_INIT (matrix), PRAND_CHUNK_LEN, PRAND_LFSR_INIT (table: the paper's 128-table
- *   jump), PRAND_MT_POLY (host: no precomputed polynomial table).  Unknown name:
+ *   jump), PRAND_MT_POLY (host: no precomputed polynomial table), PRAND_SEQ_SECTIONS (cap on the sections
+ *   of prand_generate_seq_*; not MT19937).  Unknown name:
  *   PRAND_ERR_ARG.  The launch paths read the table without a lock: call this only while no other thread is inside a
  *   libprand call (it is a test and tuning aid, not a run-time switch).
  */

@@ -137,6 +137,7 @@ struct DebugHooks {
     uint64_t chunk_len;     // PRAND_CHUNK_LEN: force the sub-section length (0: plan_chunks decides)
     bool lfsr_table;        // PRAND_LFSR_INIT=table: the paper's 128-table jump method for LFSR113
     bool mt_host_poly;      // PRAND_MT_POLY=host: compute every MT19937 jump polynomial on the host (no table)
+    uint64_t seq_sections;  // PRAND_SEQ_SECTIONS: cap on the sections of prand_generate_seq_* (0: the plan's own, 2^17)
 };
 const DebugHooks &debug_hooks();
 

@@ -78,9 +78,11 @@ void hook_assign(DebugHooks &h, const std::string &name, const char *v)
     else if (name == "PRAND_CHUNK_LEN") h.chunk_len = on ? std::strtoull(v, nullptr, 10) : 0;
     else if (name == "PRAND_LFSR_INIT") h.lfsr_table = on && std::string(v) == "table";
     else if (name == "PRAND_MT_POLY") h.mt_host_poly = on && std::string(v) == "host";
+    else if (name == "PRAND_SEQ_SECTIONS") h.seq_sections = on ? std::strtoull(v, nullptr, 10) : 0;
 }
 const char *const HOOK_NAMES[] = {"PRAND_MT_CFG", "PRAND_MT_APPLY", "PRAND_GM_LP", "PRAND_GM31_NF", "PRAND_GM_WATCH",
-                                  "PRAND_MRG_INT", "PRAND_GM_INIT", "PRAND_CHUNK_LEN", "PRAND_LFSR_INIT", "PRAND_MT_POLY"};
+                                  "PRAND_MRG_INT", "PRAND_GM_INIT", "PRAND_CHUNK_LEN", "PRAND_LFSR_INIT", "PRAND_MT_POLY",
+                                  "PRAND_SEQ_SECTIONS"};
 void hooks_from_env()
 {
     for (const char *n : HOOK_NAMES) hook_assign(g_hooks, n, std::getenv(n));
@@ -820,7 +822,8 @@ void plan_sections(int gen, uint64_t length, uint64_t *n_sections, uint64_t *sec
     const uint64_t min_len = gen == PRAND_MT19937 ? 8 * 624 : 1024;
     // MT19937: every section costs a polynomial application (~1 us of a whole SM): one CTA of four sections per SM
     // others: one section per thread; 2^17 sections are one wave of 28 warps per SM on 148 SMs
-    const uint64_t max_sec = gen == PRAND_MT19937 ? 4 * (uint64_t)sms : 131072;
+    uint64_t max_sec = gen == PRAND_MT19937 ? 4 * (uint64_t)sms : 131072;
+    if (gen != PRAND_MT19937 && debug_hooks().seq_sections) max_sec = debug_hooks().seq_sections;   // tuning hook
     uint64_t S = length / min_len;
     if (S > max_sec) S = max_sec;
     if (S < 1) S = 1;

@@ -12,7 +12,7 @@ def pytest_configure(config):
 
 
 HOOKS = ["PRAND_MT_CFG", "PRAND_MT_APPLY", "PRAND_GM_LP", "PRAND_GM31_NF", "PRAND_GM_WATCH", "PRAND_MRG_INT",
-         "PRAND_GM_INIT", "PRAND_CHUNK_LEN", "PRAND_LFSR_INIT", "PRAND_MT_POLY"]
+         "PRAND_GM_INIT", "PRAND_CHUNK_LEN", "PRAND_LFSR_INIT", "PRAND_MT_POLY", "PRAND_SEQ_SECTIONS"]
 
 import pytest  # noqa: E402
 

@@ -279,6 +279,28 @@ def test_single_sequence_fill_equals_the_serial_generator(gen):
         assert st == o.export()
 
 
+@pytest.mark.parametrize("gen", ["lfsr113", "mrg32k3a", "gm31"])
+def test_single_sequence_fill_with_other_section_counts(gen):
+    """PRAND_SEQ_SECTIONS caps the number of sections a sequence fill is cut into (tuning hook): the numbers are defined
+    by position, so any cut gives the serial generator's output and state."""
+    need_gpu()
+    seed, n = workloads.SEED.get(gen, 1), 300_007
+    want = oracle.State(gen, seed).fill(n, "u32")
+    wst = oracle.State(gen, seed).jump(n).export()
+    for cap in ("3", "64", "100000"):
+        P.prand_debug_set("PRAND_SEQ_SECTIONS", cap)
+        S, L = C.c_uint64(), C.c_uint64()
+        assert P.lib().prand_host_plan_sections(P.gen_id(gen), n, C.byref(S), C.byref(L)) == 0
+        assert S.value == min(int(cap), -(-n // L.value)) and S.value <= n // 1024      # the cap is in force
+        g = P.Generator(gen, seed, 1, 0)
+        got = g.generate_seq(n, "u32").cpu().numpy().view(np.uint32)
+        st = g.state()
+        g.close()
+        assert np.array_equal(got, want), (gen, cap)
+        assert st == wst
+    P.prand_debug_set("PRAND_SEQ_SECTIONS", None)
+
+
 def test_single_sequence_fill_needs_one_stream():
     need_gpu()
     g = P.Generator("lfsr113", 12345, 2, 1000)
