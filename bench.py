@@ -70,7 +70,8 @@ def load_alu_counts():
     if os.path.exists(path):
         with open(path, newline="") as f:
             for row in csv.DictReader(f):
-                pipes = {k: float(row[k]) for k in ("alu_pipe_pct", "fma_pipe_cycles_pct", "issue_active_pct") if row.get(k)}
+                pipes = {k: float(row[k]) for k in ("alu_pipe_pct", "fma_pipe_cycles_pct", "issue_active_pct", "fmaheavy_pipe_cycles_pct",
+                                                   "fp64_pipe_pct") if row.get(k)}
                 out[row["kernel"]] = (float(row["thread_instr_per_number"]), row["source"], pipes)
     return out
 
